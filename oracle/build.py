@@ -1,0 +1,32 @@
+"""Build the C oracle (test infrastructure) with gcc: two shared objects, fp64 and fp32.
+
+    python -m oracle.build
+
+Building the checker is not using it: __graft_entry__.build() calls this too.
+"""
+from __future__ import annotations
+
+import os
+import subprocess
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+SRC = os.path.join(HERE, "dwf_oracle.c")
+
+
+def lib_path(prec: str) -> str:
+    return os.path.join(HERE, f"liboracle_dwf_{prec}.so")
+
+
+def build(force: bool = False) -> None:
+    for prec, real in (("f64", "double"), ("f32", "float")):
+        out = lib_path(prec)
+        if not force and os.path.exists(out) and os.path.getmtime(out) >= os.path.getmtime(SRC):
+            continue
+        cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared", "-fno-fast-math",
+               f"-DORC_REAL={real}", f"-DORC_SUFFIX=_{prec}", SRC, "-o", out, "-lm"]
+        subprocess.run(cmd, check=True)
+
+
+if __name__ == "__main__":
+    build(force=True)
+    print("built", lib_path("f64"), lib_path("f32"))
