@@ -1,0 +1,145 @@
+/* dwf.h — C-ABI boundary of the B200-native domain-wall-fermion hot path (arXiv:2203.17119).
+ *
+ * What the library computes (definitions in DESIGN.md §2, readings C1-C10):
+ *   - the 4-D Wilson hopping term Dhop over all Ls fifth-dimension slices,
+ *   - the 5-D Moebius/Shamir terms (Meooe5D "A", Mooee, Mooee^-1),
+ *   - the Dirichlet-cut operator D_Omega (+) D_Omegabar (eqs. 3-4, PAPER.md:175:
+ *     "applies Dirichlet boundary conditions to its gauge field argument"),
+ *   - the red-black Schur operator Mpc and CG on Mpc^dag Mpc in fp64 and fp32-inner/fp64-outer
+ *     ("the usual red-black preconditioned HMC can be used"),
+ *   - the full-system red-black solve M psi = eta that the paper's eq. 5 Schur check needs.
+ *
+ * Conventions
+ *   Pointers named *_dev are DEVICE pointers, *_host are HOST pointers.  Field buffers are
+ *   owned by the caller (PyTorch allocates them); the context owns its gauge copies, its 5-D
+ *   coefficient tables and its solver workspace.  All work is enqueued on the context's CUDA
+ *   stream (dwf_set_stream); only dwf_cg / dwf_solve / dwf_norm2 / *_host calls synchronise
+ *   that stream, because they return scalars or host data.
+ *   Every function returns a dwf_status; nothing throws or aborts across this boundary.
+ *   dwf_last_error(ctx) gives a human-readable message for the last failure on ctx.
+ *
+ * Layouts
+ *   CANONICAL (interchange, what the oracle also uses), real type = double or float, C order:
+ *     gauge   [lex][mu][row][col][re,im]        lex = ((t*Lz+z)*Ly+y)*Lx+x, mu = 0..3 = x,y,z,t,
+ *                                               U_mu(x) is the link from x to x+mu_hat (18 reals)
+ *     FULL    [lex][s][spin][colour][re,im]
+ *     EVEN/ODD[cb][s][spin][colour][re,im]      cb = lex/2 over sites with (x+y+z+t)%2 == parity
+ *   NATIVE (opaque to the caller; dwf_field_bytes gives the size): a tiled, site-vectorised SoA,
+ *     16-byte vectors, described in DESIGN.md §4.  A FULL native field is the EVEN native field
+ *     followed by the ODD native field.
+ */
+#ifndef DWF_H
+#define DWF_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct dwf_ctx dwf_ctx; /* opaque, library-owned */
+
+typedef enum {
+    DWF_OK = 0,
+    DWF_EINVAL = 1,   /* bad argument: odd dims, Ls < 1 or > 32, cut not dividing, null/aliased pointers */
+    DWF_ENOMEM = 2,   /* device allocation failed */
+    DWF_ECUDA = 3,    /* a CUDA call or kernel launch failed */
+    DWF_ESTATE = 4,   /* gauge field not set */
+    DWF_ENOTCONV = 5  /* max_iter reached; x holds the best iterate, info is filled */
+} dwf_status;
+
+typedef enum { DWF_F32 = 0, DWF_F64 = 1 } dwf_prec;
+typedef enum { DWF_EVEN = 0, DWF_ODD = 1, DWF_FULL = 2 } dwf_parity; /* parity of the OUTPUT field */
+typedef enum { DWF_CG_F64 = 0, DWF_CG_MIXED = 1 } dwf_cg_mode;
+
+typedef struct {
+    int iters_total;     /* CG iterations, all restarts / inner solves included */
+    int iters_inner;     /* fp32 inner iterations (mixed mode), else 0 */
+    int restarts;        /* fp64: true-residual restarts; mixed: outer defect-correction steps */
+    double resid_iter;   /* recurrence residual |r|/|b| at exit */
+    double resid_true;   /* |b - A x|/|b| recomputed at exit (fp64) */
+    double resid_full;   /* dwf_solve only: |eta - M psi|/|eta| */
+    double seconds;      /* wall time of the call, enqueue to synchronise */
+    int launches;        /* kernels launched by the call */
+} dwf_cg_info;
+
+/* Create a context for an Lx*Ly*Lz*Lt lattice (all even) with Ls slices (1..32).
+ * Moebius parameters: D_+ = b5 D_W + 1, D_- = c5 D_W - 1, D_W = (4-M5) - Dhop/2 (reading C4);
+ * Shamir is (b5,c5) = (1,0).  dirichlet_cut[mu] = B > 0 (B divides L_mu) zeroes U_mu(x) for all x
+ * with x_mu mod B == B-1 (reading C7); 0 = no cut in that direction.
+ * Antiperiodic time boundary by default (reading C2). */
+dwf_status dwf_create(dwf_ctx** out, const int dims[4], int Ls, double M5, double mf, double b5, double c5,
+                      const int dirichlet_cut[4]);
+dwf_status dwf_destroy(dwf_ctx* ctx);
+
+/* Options (set before dwf_set_gauge unless noted):
+ *   "antiperiodic_t" 0/1 (default 1)       "compress12" 0/1 (default 1; 2-row links, reading C10)
+ *   "tile_x","tile_y","tile_z","tile_t"    native tile extents (default 4, or 2 where 4 does not divide)
+ *   "inner_tol" (default 1e-4), "max_restarts" (default 20)     mixed-precision CG (reading C9), any time
+ *   "dhop_sc" s-slices per thread in the Dhop kernel, "dhop_loop_s" 0/1, any time (tuning) */
+dwf_status dwf_set_option(dwf_ctx* ctx, const char* key, double val);
+dwf_status dwf_get_option(const dwf_ctx* ctx, const char* key, double* val);
+/* cudaStream_t as void* (torch.cuda.current_stream().cuda_stream); NULL = default stream */
+dwf_status dwf_set_stream(dwf_ctx* ctx, void* cuda_stream);
+
+/* Copies a canonical fp64 gauge field (device pointer, V4*4*18 doubles) into the context: applies the
+ * Dirichlet cut, builds the 8-legs-per-site native copies (forward U_mu(x), backward U_mu(x-mu)^dag) in
+ * fp64 and fp32 (round to nearest) for both parities, optionally 2-row compressed. */
+dwf_status dwf_set_gauge(dwf_ctx* ctx, const void* U_dev_canonical_f64);
+
+/* Bytes of a native field of the given precision and parity (DWF_FULL = 2 x half). */
+size_t dwf_field_bytes(const dwf_ctx* ctx, dwf_prec prec, dwf_parity parity);
+/* canonical (device, same precision) <-> native (device) */
+dwf_status dwf_pack(dwf_ctx* ctx, void* native_dev, const void* canonical_dev, dwf_prec prec, dwf_parity parity);
+dwf_status dwf_unpack(dwf_ctx* ctx, void* canonical_dev, const void* native_dev, dwf_prec prec, dwf_parity parity);
+/* native -> native precision conversion (round to nearest) */
+dwf_status dwf_convert(dwf_ctx* ctx, void* dst_dev, dwf_prec dst_prec, const void* src_dev, dwf_prec src_prec,
+                       dwf_parity parity);
+
+/* ---- operators: DEVICE pointers to NATIVE fields owned by the caller; out must not alias in ---- */
+/* Dhop psi(x,s) = sum_mu [(1-g_mu) U_mu(x) psi(x+mu,s) + (1+g_mu) U_mu(x-mu)^dag psi(x-mu,s)], reading C3;
+ * out_parity EVEN/ODD: in is the opposite-parity half field; FULL: both FULL.  dagger swaps the projectors. */
+dwf_status dwf_dhop(dwf_ctx* ctx, void* out_dev, const void* in_dev, dwf_parity out_parity, int dagger, dwf_prec prec);
+/* site-local 5-D operators (reading C5); parity only selects the field size */
+dwf_status dwf_meooe5d(dwf_ctx* ctx, void* out_dev, const void* in_dev, dwf_parity parity, int dagger, dwf_prec prec);
+dwf_status dwf_mooee(dwf_ctx* ctx, void* out_dev, const void* in_dev, dwf_parity parity, int dagger, dwf_prec prec);
+dwf_status dwf_mooee_inv(dwf_ctx* ctx, void* out_dev, const void* in_dev, dwf_parity parity, int dagger, dwf_prec prec);
+/* full unpreconditioned M = Mooee + Meooe on FULL fields (reading C4) */
+dwf_status dwf_m(dwf_ctx* ctx, void* out_dev, const void* in_dev, int dagger, dwf_prec prec);
+/* Schur operator Mpc = Moo - Moe Mee^-1 Meo on ODD fields (reading C6) */
+dwf_status dwf_mpc(dwf_ctx* ctx, void* out_dev, const void* in_dev, int dagger, dwf_prec prec);
+/* Mpc^dag Mpc on ODD fields */
+dwf_status dwf_mdagm(dwf_ctx* ctx, void* out_dev, const void* in_dev, dwf_prec prec);
+
+/* sum |v|^2 over a native field, accumulated in fp64 with a fixed reduction tree (deterministic) */
+dwf_status dwf_norm2(dwf_ctx* ctx, const void* v_dev, dwf_prec prec, dwf_parity parity, double* result_host);
+
+/* CG on Mpc^dag Mpc x = b (reading C8; mixed: C9).  x_dev: in = initial guess (use_guess != 0) else ignored,
+ * out = solution; both fp64 native ODD fields.  tol is relative to |b|.  Restarts from the true residual
+ * until |b - A x| <= tol |b|.  Returns DWF_ENOTCONV if max_iter is reached. */
+dwf_status dwf_cg(dwf_ctx* ctx, void* x_dev, const void* b_dev, double tol, int max_iter, dwf_cg_mode mode,
+                  int use_guess, dwf_cg_info* info);
+/* M psi = eta on FULL fp64 native fields through the red-black wrap (reading C6):
+ * eta' = eta_o - Moe Mee^-1 eta_e; Mpc^dag Mpc psi_o = Mpc^dag eta'; psi_e = Mee^-1 (eta_e - Meo psi_o). */
+dwf_status dwf_solve(dwf_ctx* ctx, void* psi_dev, const void* eta_dev, double tol, int max_iter, dwf_cg_mode mode,
+                     dwf_cg_info* info);
+
+/* ---- end-to-end entry points with HOST buffers in canonical layout (copies inside the call) ---- */
+/* out_host = Dhop in_host; canonical fields of the given precision */
+dwf_status dwf_dhop_host(dwf_ctx* ctx, void* out_host, const void* in_host, dwf_parity out_parity, int dagger,
+                         dwf_prec prec);
+/* out_host = Mpc^dag Mpc in_host; canonical ODD fields */
+dwf_status dwf_mdagm_host(dwf_ctx* ctx, void* out_host, const void* in_host, dwf_prec prec);
+/* psi_host = M^-1 eta_host; canonical FULL fp64 fields */
+dwf_status dwf_solve_host(dwf_ctx* ctx, void* psi_host, const void* eta_host, double tol, int max_iter,
+                          dwf_cg_mode mode, dwf_cg_info* info);
+
+/* kernels launched on this context since creation (for bench.py's gpu_launches) */
+long long dwf_launch_count(const dwf_ctx* ctx);
+const char* dwf_last_error(const dwf_ctx* ctx);
+const char* dwf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DWF_H */

@@ -1,0 +1,613 @@
+// C-ABI entry points (include/dwf.h), operator compositions and the CG drivers.
+//
+// Compositions (reading C5/C6; Meooe = -1/2 Dhop A, Mpc = Moo - Moe Mee^-1 Meo on odd sites):
+//   Mpc x     = Moo x - 1/4 Dhop_o [A Mee^-1] Dhop_e [A] x                 (5 kernels)
+//   Mpc^dag x = Moo^dag x - 1/4 A^dag Dhop^dag_o [Mee^-dag A^dag] Dhop^dag_e x   (4 kernels)
+// where [..] are single fused 5-D table kernels and the final 5-D kernel also adds the Moo term and,
+// inside CG, accumulates |Mpc p|^2.
+#include <chrono>
+#include <cmath>
+#include <cstring>
+
+#include "dwf_internal.h"
+
+using namespace dwf;
+
+namespace {
+
+const int NWS = 10;
+
+dwf_status ws_get(dwf_ctx* c, int prec, int idx, void** out) {
+    void** arr = (prec == DWF_F64) ? c->ws64 : c->ws32;
+    if (!arr[idx]) {
+        if (cudaMalloc(&arr[idx], half_bytes(c->g, prec)) != cudaSuccess) {
+            c->err = "cudaMalloc(workspace) failed";
+            cudaGetLastError();
+            return DWF_ENOMEM;
+        }
+    }
+    *out = arr[idx];
+    return DWF_OK;
+}
+
+#define DWF_TRY(expr)                       \
+    do {                                    \
+        dwf_status _s = (expr);             \
+        if (_s != DWF_OK) return _s;        \
+    } while (0)
+
+dwf_status need_gauge(dwf_ctx* c) {
+    if (!c) return DWF_EINVAL;
+    if (!c->gauge_set) { c->err = "gauge field not set (call dwf_set_gauge)"; return DWF_ESTATE; }
+    return DWF_OK;
+}
+
+size_t half_reals(const dwf_ctx* c) { return (size_t)c->g.Vh * c->g.Ls * 24; }
+
+dwf_status read_slot(dwf_ctx* c, int slot, double* v) {
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->scalars_host + slot, c->scalars + slot, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    *v = c->scalars_host[slot];
+    return DWF_OK;
+}
+
+// out = Mpc in (dagger: Mpc^dag in) on odd half fields; norm_slot >= 0 also reduces |out|^2
+dwf_status mpc_apply(dwf_ctx* c, void* out, const void* in, int dagger, int prec, int norm_slot) {
+    void *t1, *t2;
+    DWF_TRY(ws_get(c, prec, 0, &t1));
+    DWF_TRY(ws_get(c, prec, 1, &t2));
+    if (!dagger) {
+        DWF_TRY(launch_op5(c, t1, in, OP_A, nullptr, -1, 0.0, prec, -1));
+        DWF_TRY(launch_dhop(c, t2, t1, DWF_EVEN, 0, prec));
+        DWF_TRY(launch_op5(c, t1, t2, OP_A_MEEINV, nullptr, -1, 0.0, prec, -1));
+        DWF_TRY(launch_dhop(c, t2, t1, DWF_ODD, 0, prec));
+        DWF_TRY(launch_op5(c, out, in, OP_MEE, t2, -1, -0.25, prec, norm_slot));
+    } else {
+        DWF_TRY(launch_dhop(c, t1, in, DWF_EVEN, 1, prec));
+        DWF_TRY(launch_op5(c, t2, t1, OP_MEEINVDAG_ADAG, nullptr, -1, 0.0, prec, -1));
+        DWF_TRY(launch_dhop(c, t1, t2, DWF_ODD, 1, prec));
+        DWF_TRY(launch_op5(c, out, in, OP_MEEDAG, t1, OP_ADAG, -0.25, prec, norm_slot));
+    }
+    return DWF_OK;
+}
+
+dwf_status mdagm_apply(dwf_ctx* c, void* out, const void* in, int prec) {
+    void* q;
+    DWF_TRY(ws_get(c, prec, 4, &q));
+    DWF_TRY(mpc_apply(c, q, in, 0, prec, -1));
+    return mpc_apply(c, out, q, 1, prec, -1);
+}
+
+// out_p = Mpp in_p + Meooe in_(1-p) on FULL fields (even half first)
+dwf_status m_apply(dwf_ctx* c, void* out, const void* in, int dagger, int prec) {
+    void *t1, *t2;
+    DWF_TRY(ws_get(c, prec, 0, &t1));
+    DWF_TRY(ws_get(c, prec, 1, &t2));
+    const size_t hb = half_bytes(c->g, prec);
+    for (int p = 0; p < 2; ++p) {
+        const void* in_p = (const char*)in + p * hb;
+        const void* in_q = (const char*)in + (1 - p) * hb;
+        void* out_p = (char*)out + p * hb;
+        if (!dagger) {
+            DWF_TRY(launch_op5(c, t1, in_q, OP_A, nullptr, -1, 0.0, prec, -1));
+            DWF_TRY(launch_dhop(c, t2, t1, p, 0, prec));
+            DWF_TRY(launch_op5(c, out_p, in_p, OP_MEE, t2, -1, -0.5, prec, -1));
+        } else {
+            DWF_TRY(launch_dhop(c, t1, in_q, p, 1, prec));
+            DWF_TRY(launch_op5(c, out_p, in_p, OP_MEEDAG, t1, OP_ADAG, -0.5, prec, -1));
+        }
+    }
+    return DWF_OK;
+}
+
+// CG iterations on A = Mpc^dag Mpc in precision prec.  On entry r holds the residual, slot_c |r|^2 (host copy cval).
+// Mirrors the oracle's loop order (reading C8).  Returns the number of iterations done and the last |r|^2.
+dwf_status cg_iterate(dwf_ctx* c, int prec, void* x, void* r, double target, int max_iter, int* iters_io, double* cval) {
+    void *p, *q, *z;
+    DWF_TRY(ws_get(c, prec, 3, &p));
+    DWF_TRY(ws_get(c, prec, 4, &q));
+    DWF_TRY(ws_get(c, prec, 5, &z));
+    const size_t n = half_reals(c);
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(p, r, half_bytes(c->g, prec), cudaMemcpyDeviceToDevice, c->stream));
+    int slot_c = SLOT_C, slot_cn = SLOT_CN;
+    double cc = *cval;
+    while (cc > target && *iters_io < max_iter) {
+        DWF_TRY(mpc_apply(c, q, p, 0, prec, SLOT_D));                 // q = Mpc p, d = |q|^2
+        DWF_TRY(mpc_apply(c, z, q, 1, prec, -1));                     // z = Mpc^dag q
+        DWF_TRY(launch_cg_update(c, x, r, p, z, prec, n, slot_c, SLOT_D, slot_cn));
+        double cn;
+        DWF_TRY(read_slot(c, slot_cn, &cn));
+        ++*iters_io;
+        if (!(cn == cn)) { c->err = "CG: NaN residual"; *cval = cn; return DWF_ECUDA; }
+        if (cn <= target) { cc = cn; break; }
+        DWF_TRY(launch_xpay(c, p, r, prec, n, slot_cn, slot_c));      // p = r + (cn/c) p
+        int t = slot_c; slot_c = slot_cn; slot_cn = t;
+        cc = cn;
+    }
+    *cval = cc;
+    return DWF_OK;
+}
+
+dwf_status norm2_host(dwf_ctx* c, const void* v, int prec, double* out) {
+    DWF_TRY(launch_norm2(c, v, prec, half_reals(c), SLOT_T0));
+    return read_slot(c, SLOT_T0, out);
+}
+
+// r = b - A x (fp64), returns |r|^2
+dwf_status true_residual(dwf_ctx* c, void* r, const void* b, const void* x, double* rn2) {
+    void* ax;
+    DWF_TRY(ws_get(c, DWF_F64, 6, &ax));
+    DWF_TRY(mdagm_apply(c, ax, x, DWF_F64));
+    DWF_TRY(launch_sub(c, r, b, ax, DWF_F64, half_reals(c)));
+    return norm2_host(c, r, DWF_F64, rn2);
+}
+
+dwf_status cg_f64(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, int use_guess, dwf_cg_info* info) {
+    void* r;
+    DWF_TRY(ws_get(c, DWF_F64, 2, &r));
+    const size_t hb = half_bytes(c->g, DWF_F64);
+    double bn2;
+    DWF_TRY(norm2_host(c, b, DWF_F64, &bn2));
+    if (!use_guess) DWF_CUDA_CHECK(c, cudaMemsetAsync(x, 0, hb, c->stream));
+    if (bn2 == 0.0) {
+        DWF_CUDA_CHECK(c, cudaMemsetAsync(x, 0, hb, c->stream));
+        info->resid_iter = info->resid_true = 0.0;
+        return DWF_OK;
+    }
+    const double target = tol * tol * bn2;
+    int iters = 0, restarts = 0;
+    double cc = 0.0, rtrue = 0.0;
+    bool conv = false;
+    for (;;) {
+        if (use_guess || restarts > 0) {
+            DWF_TRY(true_residual(c, r, b, x, &cc));
+        } else {
+            DWF_CUDA_CHECK(c, cudaMemcpyAsync(r, b, hb, cudaMemcpyDeviceToDevice, c->stream));
+            cc = bn2;
+        }
+        c->scalars_host[SLOT_C] = cc;
+        DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->scalars + SLOT_C, c->scalars_host + SLOT_C, sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        DWF_TRY(cg_iterate(c, DWF_F64, x, r, target, max_iter, &iters, &cc));
+        info->resid_iter = std::sqrt(cc / bn2);
+        void* tr;
+        DWF_TRY(ws_get(c, DWF_F64, 7, &tr));
+        double tn2;
+        DWF_TRY(true_residual(c, tr, b, x, &tn2));
+        rtrue = std::sqrt(tn2 / bn2);
+        if (rtrue <= tol) { conv = true; break; }
+        if (iters >= max_iter) break;
+        ++restarts;
+    }
+    info->iters_total = iters;
+    info->restarts = restarts;
+    info->resid_true = rtrue;
+    return conv ? DWF_OK : DWF_ENOTCONV;
+}
+
+// reading C9: fp64 outer defect correction around an fp32 inner CG
+dwf_status cg_mixed(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, int use_guess, dwf_cg_info* info) {
+    void *r, *r32, *e32;
+    DWF_TRY(ws_get(c, DWF_F64, 2, &r));
+    DWF_TRY(ws_get(c, DWF_F32, 2, &r32));
+    DWF_TRY(ws_get(c, DWF_F32, 6, &e32));
+    const size_t hb = half_bytes(c->g, DWF_F64), hb32 = half_bytes(c->g, DWF_F32);
+    double bn2;
+    DWF_TRY(norm2_host(c, b, DWF_F64, &bn2));
+    if (!use_guess || bn2 == 0.0) DWF_CUDA_CHECK(c, cudaMemsetAsync(x, 0, hb, c->stream));
+    if (bn2 == 0.0) { info->resid_iter = info->resid_true = 0.0; return DWF_OK; }
+    int iters = 0, restarts = 0;
+    double rtrue = 0.0;
+    for (;;) {
+        double rn2;
+        DWF_TRY(true_residual(c, r, b, x, &rn2));
+        rtrue = std::sqrt(rn2 / bn2);
+        if (rtrue <= tol || restarts >= c->max_restarts || iters >= max_iter) break;
+        const double delta = std::fmax(c->inner_tol, tol * std::sqrt(bn2 / rn2));
+        DWF_TRY(launch_convert(c, r32, DWF_F32, r, DWF_F64, 1));
+        double r32n2;
+        DWF_TRY(norm2_host(c, r32, DWF_F32, &r32n2));
+        DWF_CUDA_CHECK(c, cudaMemsetAsync(e32, 0, hb32, c->stream));
+        c->scalars_host[SLOT_C] = r32n2;
+        DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->scalars + SLOT_C, c->scalars_host + SLOT_C, sizeof(double), cudaMemcpyHostToDevice, c->stream));
+        double cc = r32n2;
+        DWF_TRY(cg_iterate(c, DWF_F32, e32, r32, delta * delta * r32n2, max_iter, &iters, &cc));
+        info->resid_iter = std::sqrt(cc / r32n2);
+        DWF_TRY(launch_add_f32_to_f64(c, x, e32, 0));
+        ++restarts;
+    }
+    info->iters_total = iters;
+    info->iters_inner = iters;
+    info->restarts = restarts;
+    info->resid_true = rtrue;
+    return (rtrue <= tol) ? DWF_OK : DWF_ENOTCONV;
+}
+
+double now_s() {
+    return std::chrono::duration<double>(std::chrono::steady_clock::now().time_since_epoch()).count();
+}
+
+dwf_status stage_get(dwf_ctx* c, int idx, size_t bytes, void** out) {
+    if (c->stage_bytes[idx] < bytes) {
+        if (c->stage_dev[idx]) cudaFree(c->stage_dev[idx]);
+        c->stage_dev[idx] = nullptr;
+        c->stage_bytes[idx] = 0;
+        if (cudaMalloc(&c->stage_dev[idx], bytes) != cudaSuccess) { c->err = "cudaMalloc(stage) failed"; cudaGetLastError(); return DWF_ENOMEM; }
+        c->stage_bytes[idx] = bytes;
+    }
+    *out = c->stage_dev[idx];
+    return DWF_OK;
+}
+
+void choose_tiles(dwf_ctx* c) {
+    Geom& g = c->g;
+    for (int mu = 0; mu < 4; ++mu) {
+        int t = c->tile_opt[mu];
+        if (t <= 0) t = (g.L[mu] % 4 == 0) ? 4 : 2;
+        g.T[mu] = t;
+        g.NT[mu] = g.L[mu] / t;
+    }
+    g.TS = g.T[0] * g.T[1] * g.T[2] * g.T[3] / 2;
+    g.ntiles = g.NT[0] * g.NT[1] * g.NT[2] * g.NT[3];
+    g.Vh = g.ntiles * g.TS;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* dwf_version(void) { return "dwf_b200 0.1 (sm_100a)"; }
+
+dwf_status dwf_create(dwf_ctx** out, const int dims[4], int Ls, double M5, double mf, double b5, double c5,
+                      const int dirichlet_cut[4]) {
+    if (!out || !dims) return DWF_EINVAL;
+    *out = nullptr;
+    if (Ls < 1 || Ls > 32) return DWF_EINVAL;
+    long long V = 1;
+    for (int mu = 0; mu < 4; ++mu) {
+        if (dims[mu] < 2 || (dims[mu] & 1)) return DWF_EINVAL;
+        if (dirichlet_cut) {
+            int B = dirichlet_cut[mu];
+            if (B < 0 || (B > 0 && dims[mu] % B != 0)) return DWF_EINVAL;
+        }
+        V *= dims[mu];
+    }
+    if (V / 2 * Ls * 12 >= (1LL << 31)) return DWF_EINVAL;   // 32-bit vector indices inside the kernels
+    const double bee = 1.0 + b5 * (4.0 - M5);
+    if (bee == 0.0) return DWF_EINVAL;
+    dwf_ctx* c = new (std::nothrow) dwf_ctx();
+    if (!c) return DWF_ENOMEM;
+    for (int mu = 0; mu < 4; ++mu) {
+        c->g.L[mu] = dims[mu];
+        c->cut[mu] = dirichlet_cut ? dirichlet_cut[mu] : 0;
+    }
+    c->g.Ls = Ls;
+    c->g.antiperiodic_t = 1;
+    c->M5 = M5; c->mf = mf; c->b5 = b5; c->c5 = c5;
+    choose_tiles(c);
+    build_tables(c);
+    if (cudaMalloc(&c->scalars, sizeof(double) * NSLOTS) != cudaSuccess ||
+        cudaMallocHost(&c->scalars_host, sizeof(double) * NSLOTS) != cudaSuccess) {
+        cudaGetLastError();
+        delete c;
+        return DWF_ECUDA;
+    }
+    cudaMemset(c->scalars, 0, sizeof(double) * NSLOTS);
+    // device tables [op][chirality][Ls*Ls]
+    const size_t nt = (size_t)OP5_COUNT * 2 * Ls * Ls;
+    std::vector<double> h64(nt);
+    std::vector<float> h32(nt);
+    for (int op = 0; op < OP5_COUNT; ++op)
+        for (int ch = 0; ch < 2; ++ch)
+            for (int s = 0; s < Ls; ++s)
+                for (int t = 0; t < Ls; ++t) {
+                    const double v = (ch == 0 ? c->tab[op].p : c->tab[op].m)[s * 32 + t];
+                    const size_t i = (((size_t)op * 2 + ch) * Ls + s) * Ls + t;
+                    h64[i] = v;
+                    h32[i] = (float)v;
+                }
+    if (cudaMalloc(&c->dtab.d64, nt * sizeof(double)) != cudaSuccess || cudaMalloc(&c->dtab.d32, nt * sizeof(float)) != cudaSuccess) {
+        cudaGetLastError();
+        dwf_destroy(c);
+        return DWF_ENOMEM;
+    }
+    cudaMemcpy(c->dtab.d64, h64.data(), nt * sizeof(double), cudaMemcpyHostToDevice);
+    cudaMemcpy(c->dtab.d32, h32.data(), nt * sizeof(float), cudaMemcpyHostToDevice);
+    if (cudaGetLastError() != cudaSuccess) { dwf_destroy(c); return DWF_ECUDA; }
+    *out = c;
+    return DWF_OK;
+}
+
+dwf_status dwf_destroy(dwf_ctx* c) {
+    if (!c) return DWF_EINVAL;
+    for (int p = 0; p < 2; ++p) {
+        if (c->W64[p]) cudaFree(c->W64[p]);
+        if (c->W32[p]) cudaFree(c->W32[p]);
+        if (c->stage_dev[p]) cudaFree(c->stage_dev[p]);
+    }
+    for (int i = 0; i < NWS; ++i) {
+        if (c->ws64[i]) cudaFree(c->ws64[i]);
+        if (c->ws32[i]) cudaFree(c->ws32[i]);
+    }
+    if (c->partials) cudaFree(c->partials);
+    if (c->scalars) cudaFree(c->scalars);
+    if (c->scalars_host) cudaFreeHost(c->scalars_host);
+    if (c->dtab.d64) cudaFree(c->dtab.d64);
+    if (c->dtab.d32) cudaFree(c->dtab.d32);
+    cudaGetLastError();
+    delete c;
+    return DWF_OK;
+}
+
+dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
+    if (!c || !key) return DWF_EINVAL;
+    const std::string k(key);
+    const bool pre_gauge = (k == "antiperiodic_t" || k == "compress12" || k.rfind("tile_", 0) == 0);
+    if (pre_gauge && c->gauge_set) { c->err = "option '" + k + "' must be set before dwf_set_gauge"; return DWF_ESTATE; }
+    if (k == "antiperiodic_t") c->g.antiperiodic_t = (val != 0.0);
+    else if (k == "compress12") c->compress12 = (val != 0.0);
+    else if (k == "tile_x" || k == "tile_y" || k == "tile_z" || k == "tile_t") {
+        const int mu = (k == "tile_x") ? 0 : (k == "tile_y") ? 1 : (k == "tile_z") ? 2 : 3;
+        const int t = (int)val;
+        if (t < 1 || c->g.L[mu] % t != 0 || (mu == 0 && (t & 1))) { c->err = "bad tile extent"; return DWF_EINVAL; }
+        const int old = c->tile_opt[mu];
+        c->tile_opt[mu] = t;
+        choose_tiles(c);
+        if (c->g.TS > 1024) { c->tile_opt[mu] = old; choose_tiles(c); c->err = "tile too large"; return DWF_EINVAL; }
+    } else if (k == "inner_tol") c->inner_tol = val;
+    else if (k == "max_restarts") c->max_restarts = (int)val;
+    else if (k == "dhop_sc") { if (val < 0 || val > 4) return DWF_EINVAL; c->dhop_sc = (int)val; }
+    else if (k == "dhop_loop_s") c->dhop_loop_s = (val != 0.0);
+    else { c->err = "unknown option '" + k + "'"; return DWF_EINVAL; }
+    return DWF_OK;
+}
+
+dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
+    if (!c || !key || !val) return DWF_EINVAL;
+    const std::string k(key);
+    if (k == "antiperiodic_t") *val = c->g.antiperiodic_t;
+    else if (k == "compress12") *val = c->compress12;
+    else if (k == "tile_x") *val = c->g.T[0];
+    else if (k == "tile_y") *val = c->g.T[1];
+    else if (k == "tile_z") *val = c->g.T[2];
+    else if (k == "tile_t") *val = c->g.T[3];
+    else if (k == "inner_tol") *val = c->inner_tol;
+    else if (k == "max_restarts") *val = c->max_restarts;
+    else if (k == "dhop_sc") *val = c->dhop_sc;
+    else if (k == "dhop_loop_s") *val = c->dhop_loop_s;
+    else return DWF_EINVAL;
+    return DWF_OK;
+}
+
+dwf_status dwf_set_stream(dwf_ctx* c, void* s) {
+    if (!c) return DWF_EINVAL;
+    c->stream = (cudaStream_t)s;
+    return DWF_OK;
+}
+
+dwf_status dwf_set_gauge(dwf_ctx* c, const void* U) {
+    if (!c || !U) return DWF_EINVAL;
+    const Geom& g = c->g;
+    const int ng = c->compress12 ? 12 : 18;
+    const size_t b64 = (size_t)g.Vh * 8 * ((ng + 1) / 2) * 16, b32 = (size_t)g.Vh * 8 * ((ng + 3) / 4) * 16;
+    for (int p = 0; p < 2; ++p) {
+        if (c->W64[p] && c->wbytes64 != b64) { cudaFree(c->W64[p]); c->W64[p] = nullptr; }
+        if (c->W32[p] && c->wbytes32 != b32) { cudaFree(c->W32[p]); c->W32[p] = nullptr; }
+        if (!c->W64[p] && cudaMalloc(&c->W64[p], b64) != cudaSuccess) { cudaGetLastError(); c->err = "cudaMalloc(gauge) failed"; return DWF_ENOMEM; }
+        if (!c->W32[p] && cudaMalloc(&c->W32[p], b32) != cudaSuccess) { cudaGetLastError(); c->err = "cudaMalloc(gauge) failed"; return DWF_ENOMEM; }
+    }
+    c->wbytes64 = b64;
+    c->wbytes32 = b32;
+    DWF_TRY(launch_gauge_prep(c, (const double*)U));
+    c->gauge_set = true;
+    return DWF_OK;
+}
+
+size_t dwf_field_bytes(const dwf_ctx* c, dwf_prec prec, dwf_parity parity) {
+    if (!c) return 0;
+    return half_bytes(c->g, prec) * (parity == DWF_FULL ? 2 : 1);
+}
+
+dwf_status dwf_pack(dwf_ctx* c, void* native, const void* canon, dwf_prec prec, dwf_parity parity) {
+    if (!c || !native || !canon) return DWF_EINVAL;
+    return launch_pack(c, native, canon, prec, parity, false);
+}
+dwf_status dwf_unpack(dwf_ctx* c, void* canon, const void* native, dwf_prec prec, dwf_parity parity) {
+    if (!c || !native || !canon) return DWF_EINVAL;
+    return launch_pack(c, const_cast<void*>(native), canon, prec, parity, true);
+}
+dwf_status dwf_convert(dwf_ctx* c, void* dst, dwf_prec dp, const void* src, dwf_prec sp, dwf_parity parity) {
+    if (!c || !dst || !src || dst == src) return DWF_EINVAL;
+    return launch_convert(c, dst, dp, src, sp, parity == DWF_FULL ? 2 : 1);
+}
+
+dwf_status dwf_dhop(dwf_ctx* c, void* out, const void* in, dwf_parity out_parity, int dagger, dwf_prec prec) {
+    DWF_TRY(need_gauge(c));
+    if (!out || !in || out == in) { c->err = "dhop: null or aliased pointers"; return DWF_EINVAL; }
+    if (out_parity == DWF_FULL) {
+        const size_t hb = half_bytes(c->g, prec);
+        DWF_TRY(launch_dhop(c, out, (const char*)in + hb, DWF_EVEN, dagger, prec));
+        return launch_dhop(c, (char*)out + hb, in, DWF_ODD, dagger, prec);
+    }
+    return launch_dhop(c, out, in, out_parity, dagger, prec);
+}
+
+static dwf_status op5_public(dwf_ctx* c, void* out, const void* in, dwf_parity parity, int op, dwf_prec prec) {
+    if (!c || !out || !in) return DWF_EINVAL;
+    if (out == in) { c->err = "5-D operator: out must not alias in"; return DWF_EINVAL; }
+    const int nh = (parity == DWF_FULL) ? 2 : 1;
+    const size_t hb = half_bytes(c->g, prec);
+    for (int h = 0; h < nh; ++h) DWF_TRY(launch_op5(c, (char*)out + h * hb, (const char*)in + h * hb, op, nullptr, -1, 0.0, prec, -1));
+    return DWF_OK;
+}
+dwf_status dwf_meooe5d(dwf_ctx* c, void* out, const void* in, dwf_parity par, int dagger, dwf_prec prec) {
+    return op5_public(c, out, in, par, dagger ? OP_ADAG : OP_A, prec);
+}
+dwf_status dwf_mooee(dwf_ctx* c, void* out, const void* in, dwf_parity par, int dagger, dwf_prec prec) {
+    return op5_public(c, out, in, par, dagger ? OP_MEEDAG : OP_MEE, prec);
+}
+dwf_status dwf_mooee_inv(dwf_ctx* c, void* out, const void* in, dwf_parity par, int dagger, dwf_prec prec) {
+    return op5_public(c, out, in, par, dagger ? OP_MEEINVDAG : OP_MEEINV, prec);
+}
+
+dwf_status dwf_m(dwf_ctx* c, void* out, const void* in, int dagger, dwf_prec prec) {
+    DWF_TRY(need_gauge(c));
+    if (!out || !in || out == in) { c->err = "m: null or aliased pointers"; return DWF_EINVAL; }
+    return m_apply(c, out, in, dagger, prec);
+}
+dwf_status dwf_mpc(dwf_ctx* c, void* out, const void* in, int dagger, dwf_prec prec) {
+    DWF_TRY(need_gauge(c));
+    if (!out || !in || out == in) { c->err = "mpc: null or aliased pointers"; return DWF_EINVAL; }
+    return mpc_apply(c, out, in, dagger, prec, -1);
+}
+dwf_status dwf_mdagm(dwf_ctx* c, void* out, const void* in, dwf_prec prec) {
+    DWF_TRY(need_gauge(c));
+    if (!out || !in || out == in) { c->err = "mdagm: null or aliased pointers"; return DWF_EINVAL; }
+    return mdagm_apply(c, out, in, prec);
+}
+
+dwf_status dwf_norm2(dwf_ctx* c, const void* v, dwf_prec prec, dwf_parity parity, double* result) {
+    if (!c || !v || !result) return DWF_EINVAL;
+    const size_t n = half_reals(c) * (parity == DWF_FULL ? 2 : 1);
+    DWF_TRY(launch_norm2(c, v, prec, n, SLOT_T0));
+    return read_slot(c, SLOT_T0, result);
+}
+
+dwf_status dwf_cg(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, dwf_cg_mode mode, int use_guess,
+                  dwf_cg_info* info) {
+    DWF_TRY(need_gauge(c));
+    dwf_cg_info local;
+    if (!info) info = &local;
+    memset(info, 0, sizeof(*info));
+    if (!x || !b || x == b || tol <= 0.0 || max_iter < 0) { c->err = "cg: bad arguments"; return DWF_EINVAL; }
+    const long long l0 = c->launches;
+    const double t0 = now_s();
+    dwf_status st = (mode == DWF_CG_MIXED) ? cg_mixed(c, x, b, tol, max_iter, use_guess, info)
+                                           : cg_f64(c, x, b, tol, max_iter, use_guess, info);
+    cudaStreamSynchronize(c->stream);
+    info->seconds = now_s() - t0;
+    info->launches = (int)(c->launches - l0);
+    if (st == DWF_ENOTCONV) c->err = "cg: max_iter reached";
+    return st;
+}
+
+dwf_status dwf_solve(dwf_ctx* c, void* psi, const void* eta, double tol, int max_iter, dwf_cg_mode mode, dwf_cg_info* info) {
+    DWF_TRY(need_gauge(c));
+    dwf_cg_info local;
+    if (!info) info = &local;
+    memset(info, 0, sizeof(*info));
+    if (!psi || !eta || psi == eta || tol <= 0.0) { c->err = "solve: bad arguments"; return DWF_EINVAL; }
+    const long long l0 = c->launches;
+    const double t0 = now_s();
+    const int P = DWF_F64;
+    const size_t hb = half_bytes(c->g, P);
+    const void* eta_e = eta;
+    const void* eta_o = (const char*)eta + hb;
+    void* psi_e = psi;
+    void* psi_o = (char*)psi + hb;
+    void *t1, *t2, *src, *rhs;
+    DWF_TRY(ws_get(c, P, 0, &t1));
+    DWF_TRY(ws_get(c, P, 1, &t2));
+    DWF_TRY(ws_get(c, P, 8, &src));
+    DWF_TRY(ws_get(c, P, 9, &rhs));
+    // src = eta_o - Moe Mee^-1 eta_e = eta_o + 1/2 Dhop_o A Mee^-1 eta_e
+    DWF_TRY(launch_op5(c, t1, eta_e, OP_A_MEEINV, nullptr, -1, 0.0, P, -1));
+    DWF_TRY(launch_dhop(c, t2, t1, DWF_ODD, 0, P));
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(src, eta_o, hb, cudaMemcpyDeviceToDevice, c->stream));
+    DWF_TRY(launch_axpy(c, src, t2, 0.5, P, half_reals(c)));
+    DWF_TRY(mpc_apply(c, rhs, src, 1, P, -1));
+    dwf_status st = (mode == DWF_CG_MIXED) ? cg_mixed(c, psi_o, rhs, tol, max_iter, 0, info)
+                                           : cg_f64(c, psi_o, rhs, tol, max_iter, 0, info);
+    if (st != DWF_OK && st != DWF_ENOTCONV) return st;
+    // psi_e = Mee^-1 (eta_e - Meo psi_o) = Mee^-1 (eta_e + 1/2 Dhop_e A psi_o)
+    DWF_TRY(launch_op5(c, t1, psi_o, OP_A, nullptr, -1, 0.0, P, -1));
+    DWF_TRY(launch_dhop(c, t2, t1, DWF_EVEN, 0, P));
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(t1, eta_e, hb, cudaMemcpyDeviceToDevice, c->stream));
+    DWF_TRY(launch_axpy(c, t1, t2, 0.5, P, half_reals(c)));
+    DWF_TRY(launch_op5(c, psi_e, t1, OP_MEEINV, nullptr, -1, 0.0, P, -1));
+    // |eta - M psi| / |eta|
+    void *me, *mo;
+    DWF_TRY(ws_get(c, P, 2, &me));
+    DWF_TRY(ws_get(c, P, 3, &mo));
+    double en2 = 0, rn2 = 0, v;
+    for (int p = 0; p < 2; ++p) {
+        const void* in_p = (const char*)psi + p * hb;
+        const void* in_q = (const char*)psi + (1 - p) * hb;
+        const void* e_p = (const char*)eta + p * hb;
+        DWF_TRY(launch_op5(c, t1, in_q, OP_A, nullptr, -1, 0.0, P, -1));
+        DWF_TRY(launch_dhop(c, t2, t1, p, 0, P));
+        DWF_TRY(launch_op5(c, me, in_p, OP_MEE, t2, -1, -0.5, P, -1));
+        DWF_TRY(launch_sub(c, mo, e_p, me, P, half_reals(c)));
+        DWF_TRY(norm2_host(c, mo, P, &v)); rn2 += v;
+        DWF_TRY(norm2_host(c, e_p, P, &v)); en2 += v;
+    }
+    info->resid_full = (en2 > 0) ? std::sqrt(rn2 / en2) : 0.0;
+    cudaStreamSynchronize(c->stream);
+    info->seconds = now_s() - t0;
+    info->launches = (int)(c->launches - l0);
+    return st;
+}
+
+dwf_status dwf_dhop_host(dwf_ctx* c, void* out_host, const void* in_host, dwf_parity out_parity, int dagger, dwf_prec prec) {
+    DWF_TRY(need_gauge(c));
+    if (!out_host || !in_host) return DWF_EINVAL;
+    const size_t nb = dwf_field_bytes(c, prec, out_parity);
+    void *canon, *nat;
+    DWF_TRY(stage_get(c, 0, nb, &canon));
+    DWF_TRY(stage_get(c, 1, 2 * nb, &nat));
+    void* nat_in = nat;
+    void* nat_out = (char*)nat + nb;
+    const dwf_parity in_par = (out_parity == DWF_FULL) ? DWF_FULL : (out_parity == DWF_EVEN ? DWF_ODD : DWF_EVEN);
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(canon, in_host, nb, cudaMemcpyHostToDevice, c->stream));
+    DWF_TRY(launch_pack(c, nat_in, canon, prec, in_par, false));
+    DWF_TRY(dwf_dhop(c, nat_out, nat_in, out_parity, dagger, prec));
+    DWF_TRY(launch_pack(c, nat_out, canon, prec, out_parity, true));
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(out_host, canon, nb, cudaMemcpyDeviceToHost, c->stream));
+    DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return DWF_OK;
+}
+
+dwf_status dwf_mdagm_host(dwf_ctx* c, void* out_host, const void* in_host, dwf_prec prec) {
+    DWF_TRY(need_gauge(c));
+    if (!out_host || !in_host) return DWF_EINVAL;
+    const size_t nb = dwf_field_bytes(c, prec, DWF_ODD);
+    void *canon, *nat;
+    DWF_TRY(stage_get(c, 0, nb, &canon));
+    DWF_TRY(stage_get(c, 1, 2 * nb, &nat));
+    void* nat_in = nat;
+    void* nat_out = (char*)nat + nb;
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(canon, in_host, nb, cudaMemcpyHostToDevice, c->stream));
+    DWF_TRY(launch_pack(c, nat_in, canon, prec, DWF_ODD, false));
+    DWF_TRY(mdagm_apply(c, nat_out, nat_in, prec));
+    DWF_TRY(launch_pack(c, nat_out, canon, prec, DWF_ODD, true));
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(out_host, canon, nb, cudaMemcpyDeviceToHost, c->stream));
+    DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    return DWF_OK;
+}
+
+dwf_status dwf_solve_host(dwf_ctx* c, void* psi_host, const void* eta_host, double tol, int max_iter, dwf_cg_mode mode,
+                          dwf_cg_info* info) {
+    DWF_TRY(need_gauge(c));
+    if (!psi_host || !eta_host) return DWF_EINVAL;
+    const double t0 = now_s();
+    const long long l0 = c->launches;
+    const size_t nb = dwf_field_bytes(c, DWF_F64, DWF_FULL);
+    void *canon, *nat;
+    DWF_TRY(stage_get(c, 0, nb, &canon));
+    DWF_TRY(stage_get(c, 1, 2 * nb, &nat));
+    void* nat_eta = nat;
+    void* nat_psi = (char*)nat + nb;
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(canon, eta_host, nb, cudaMemcpyHostToDevice, c->stream));
+    DWF_TRY(launch_pack(c, nat_eta, canon, DWF_F64, DWF_FULL, false));
+    dwf_status st = dwf_solve(c, nat_psi, nat_eta, tol, max_iter, mode, info);
+    if (st != DWF_OK && st != DWF_ENOTCONV) return st;
+    DWF_TRY(launch_pack(c, nat_psi, canon, DWF_F64, DWF_FULL, true));
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(psi_host, canon, nb, cudaMemcpyDeviceToHost, c->stream));
+    DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (info) { info->seconds = now_s() - t0; info->launches = (int)(c->launches - l0); }
+    return st;
+}
+
+long long dwf_launch_count(const dwf_ctx* c) { return c ? c->launches : 0; }
+const char* dwf_last_error(const dwf_ctx* c) { return c ? c->err.c_str() : "null context"; }
+
+}  // extern "C"

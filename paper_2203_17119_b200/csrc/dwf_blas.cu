@@ -1,0 +1,171 @@
+// BLAS-1 kernels of the CG (reading C8): 128-bit grid-stride streaming with the norm fused into the
+// update kernel; every reduction is accumulated in fp64 through warp shuffles -> one partial per block ->
+// a fixed-tree single-block pass (deterministic: the same inputs always give the same bits).
+// CG scalars stay on the device: alpha = c/d and beta = c'/c are formed inside the kernels from the
+// scalar slots, so the host only reads one double per iteration for the stopping test.
+#include "dwf_internal.h"
+
+namespace dwf {
+
+dwf_status ensure_partials(dwf_ctx* c, int n);
+dwf_status launch_reduce(dwf_ctx* c, int n, int slot);
+
+template <typename R> struct VB;
+template <> struct VB<float> { using V = float4; static constexpr int VW = 4; };
+template <> struct VB<double> { using V = double2; static constexpr int VW = 2; };
+
+__device__ __forceinline__ double blk_sum(double v) {
+    __shared__ double wsum[32];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    if (l == 0) wsum[w] = v;
+    __syncthreads();
+    const int nw = (blockDim.x + 31) >> 5;
+    v = (threadIdx.x < nw) ? wsum[threadIdx.x] : 0.0;
+    if (w == 0) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    }
+    return v;
+}
+
+__device__ __forceinline__ double n2(const float4& a) {
+    return (double)a.x * a.x + (double)a.y * a.y + (double)a.z * a.z + (double)a.w * a.w;
+}
+__device__ __forceinline__ double n2(const double2& a) { return a.x * a.x + a.y * a.y; }
+__device__ __forceinline__ float4 axpyv(float a, const float4& x, const float4& y) {
+    return make_float4(fmaf(a, x.x, y.x), fmaf(a, x.y, y.y), fmaf(a, x.z, y.z), fmaf(a, x.w, y.w));
+}
+__device__ __forceinline__ double2 axpyv(double a, const double2& x, const double2& y) {
+    return make_double2(fma(a, x.x, y.x), fma(a, x.y, y.y));
+}
+
+template <typename R>
+__global__ void __launch_bounds__(256) norm2_kernel(const typename VB<R>::V* __restrict__ v, size_t nvec,
+                                                    double* __restrict__ partials) {
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x)
+        acc += n2(v[i]);
+    double tot = blk_sum(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+}
+
+// x += a p ; r -= a z ; partial |r|^2 ;  a = sc[slot_c]/sc[slot_d]
+template <typename R>
+__global__ void __launch_bounds__(256) cg_update_kernel(typename VB<R>::V* __restrict__ x, typename VB<R>::V* __restrict__ r,
+                                                        const typename VB<R>::V* __restrict__ p,
+                                                        const typename VB<R>::V* __restrict__ z, size_t nvec,
+                                                        const double* __restrict__ sc, int slot_c, int slot_d,
+                                                        double* __restrict__ partials) {
+    const R a = (R)(sc[slot_c] / sc[slot_d]);
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        x[i] = axpyv(a, p[i], x[i]);
+        typename VB<R>::V rn = axpyv(-a, z[i], r[i]);
+        r[i] = rn;
+        acc += n2(rn);
+    }
+    double tot = blk_sum(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+}
+
+// p = r + b p ; b = sc[slot_cn]/sc[slot_c]
+template <typename R>
+__global__ void __launch_bounds__(256) xpay_kernel(typename VB<R>::V* __restrict__ p, const typename VB<R>::V* __restrict__ r,
+                                                   size_t nvec, const double* __restrict__ sc, int slot_cn, int slot_c) {
+    const R b = (R)(sc[slot_cn] / sc[slot_c]);
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x)
+        p[i] = axpyv(b, p[i], r[i]);
+}
+
+// y += a x
+template <typename R>
+__global__ void __launch_bounds__(256) axpy_kernel(typename VB<R>::V* __restrict__ y, const typename VB<R>::V* __restrict__ x,
+                                                   R a, size_t nvec) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x)
+        y[i] = axpyv(a, x[i], y[i]);
+}
+
+// out = a - b
+template <typename R>
+__global__ void __launch_bounds__(256) sub_kernel(typename VB<R>::V* __restrict__ out, const typename VB<R>::V* __restrict__ a,
+                                                  const typename VB<R>::V* __restrict__ b, size_t nvec) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x)
+        out[i] = axpyv((R)-1, b[i], a[i]);
+}
+
+static inline int blas_grid(size_t nvec) {
+    size_t want = (nvec + 255) / 256;
+    size_t cap = 148 * 8;                    // 8 CTAs of 256 threads per SM, one wave
+    return (int)(want < cap ? (want ? want : 1) : cap);
+}
+
+#define DWF_BLAS_DISPATCH(prec, CALL32, CALL64) \
+    do { if ((prec) == DWF_F64) { CALL64; } else { CALL32; } } while (0)
+
+dwf_status launch_norm2(dwf_ctx* c, const void* v, int prec, size_t nreal, int slot) {
+    const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
+    const int grid = blas_grid(nvec);
+    dwf_status st = ensure_partials(c, grid);
+    if (st != DWF_OK) return st;
+    DWF_BLAS_DISPATCH(prec, (norm2_kernel<float><<<grid, 256, 0, c->stream>>>((const float4*)v, nvec, c->partials)),
+                      (norm2_kernel<double><<<grid, 256, 0, c->stream>>>((const double2*)v, nvec, c->partials)));
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return launch_reduce(c, grid, slot);
+}
+
+dwf_status launch_cg_update(dwf_ctx* c, void* x, void* r, const void* p, const void* z, int prec, size_t nreal,
+                            int slot_c, int slot_d, int slot_cn) {
+    const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
+    const int grid = blas_grid(nvec);
+    dwf_status st = ensure_partials(c, grid);
+    if (st != DWF_OK) return st;
+    DWF_BLAS_DISPATCH(prec,
+                      (cg_update_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)x, (float4*)r, (const float4*)p,
+                                                                          (const float4*)z, nvec, c->scalars, slot_c,
+                                                                          slot_d, c->partials)),
+                      (cg_update_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)x, (double2*)r, (const double2*)p,
+                                                                           (const double2*)z, nvec, c->scalars, slot_c,
+                                                                           slot_d, c->partials)));
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return launch_reduce(c, grid, slot_cn);
+}
+
+dwf_status launch_xpay(dwf_ctx* c, void* p, const void* r, int prec, size_t nreal, int slot_cn, int slot_c) {
+    const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
+    const int grid = blas_grid(nvec);
+    DWF_BLAS_DISPATCH(prec,
+                      (xpay_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)p, (const float4*)r, nvec, c->scalars,
+                                                                     slot_cn, slot_c)),
+                      (xpay_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)p, (const double2*)r, nvec, c->scalars,
+                                                                      slot_cn, slot_c)));
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
+}
+
+dwf_status launch_axpy(dwf_ctx* c, void* y, const void* x, double a, int prec, size_t nreal) {
+    const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
+    const int grid = blas_grid(nvec);
+    DWF_BLAS_DISPATCH(prec, (axpy_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)y, (const float4*)x, (float)a, nvec)),
+                      (axpy_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)y, (const double2*)x, a, nvec)));
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
+}
+
+dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int prec, size_t nreal) {
+    const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
+    const int grid = blas_grid(nvec);
+    DWF_BLAS_DISPATCH(prec,
+                      (sub_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)out, (const float4*)a, (const float4*)b, nvec)),
+                      (sub_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)out, (const double2*)a, (const double2*)b, nvec)));
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
+}
+
+}  // namespace dwf

@@ -1,0 +1,170 @@
+// Gauge preparation (step a0) and layout conversion kernels.
+//
+// Gauge prep implements PAPER.md:175 ("applies Dirichlet boundary conditions to its gauge field
+// argument", reading C7): every link with x_mu mod B == B-1 is zeroed, then each OUTPUT site gets its 8
+// leg matrices W_leg(x): forward U_mu(x), backward U_mu(x-mu)^dag, so that the hopping kernel reads all
+// its links from its own lane (coalesced) and multiplies every leg the same way.  2-row compression
+// (reading C10) keeps rows 0,1 of W; the antiperiodic sign is NOT baked in (it would be lost by the
+// row-2 reconstruction) and is applied in the hopping kernel.
+#include "dwf_layout.cuh"
+
+namespace dwf {
+
+template <typename R>
+__global__ void gauge_prep_kernel(Geom g, const double* __restrict__ U, R* __restrict__ W, int parity, int ng,
+                                  int kg_vw /* reals per link in the native array: KG*VW */, int vw, int cut0, int cut1,
+                                  int cut2, int cut3) {
+    const int gid = blockIdx.x * blockDim.x + threadIdx.x;      // (native site, leg)
+    if (gid >= g.Vh * 8) return;
+    const int leg = gid & 7, site = gid >> 3;
+    const int tile = site / g.TS, lane = site - tile * g.TS;
+    const int mu = leg >> 1, dir = leg & 1;
+    const int cut[4] = {cut0, cut1, cut2, cut3};
+    Coord c = site_coords(g, tile, lane, parity);
+    int y[4] = {c.x[0], c.x[1], c.x[2], c.x[3]};
+    if (dir == 1) { y[mu] = c.x[mu] - 1; if (y[mu] < 0) y[mu] = g.L[mu] - 1; }
+    const double* u = U + (lex_index(g, y) * 4 + mu) * 18;
+    const bool zero = (cut[mu] > 0) && (y[mu] % cut[mu] == cut[mu] - 1);
+    double w[18];
+#pragma unroll
+    for (int r = 0; r < 3; ++r)
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) {
+            double re, im;
+            if (dir == 0) { re = u[(r * 3 + cc) * 2]; im = u[(r * 3 + cc) * 2 + 1]; }
+            else          { re = u[(cc * 3 + r) * 2]; im = -u[(cc * 3 + r) * 2 + 1]; }
+            w[(r * 3 + cc) * 2] = zero ? 0.0 : re;
+            w[(r * 3 + cc) * 2 + 1] = zero ? 0.0 : im;
+        }
+    // native: real index = (((tile*8 + leg)*KG + kg)*TS + lane)*VW + j, with i = kg*VW + j
+    const int KG = kg_vw / vw;
+    R* base = W + ((size_t)(tile * 8 + leg) * KG) * g.TS * vw;
+    for (int i = 0; i < kg_vw; ++i) {
+        const int kg = i / vw, j = i - kg * vw;
+        base[((size_t)kg * g.TS + lane) * vw + j] = (i < ng) ? (R)w[i] : (R)0;
+    }
+}
+
+dwf_status launch_gauge_prep(dwf_ctx* c, const double* Ucanon) {
+    const Geom& g = c->g;
+    const int ng = c->compress12 ? 12 : 18;
+    const int block = 128, grid = (g.Vh * 8 + block - 1) / block;
+    for (int par = 0; par < 2; ++par) {
+        const int kg64 = (ng + 1) / 2 * 2, kg32 = (ng + 3) / 4 * 4;
+        gauge_prep_kernel<double><<<grid, block, 0, c->stream>>>(g, Ucanon, (double*)c->W64[par], par, ng, kg64, 2,
+                                                                 c->cut[0], c->cut[1], c->cut[2], c->cut[3]);
+        gauge_prep_kernel<float><<<grid, block, 0, c->stream>>>(g, Ucanon, (float*)c->W32[par], par, ng, kg32, 4,
+                                                                c->cut[0], c->cut[1], c->cut[2], c->cut[3]);
+        c->launches += 2;
+    }
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
+}
+
+// ---- spinor layout conversion: canonical <-> native, native f32 <-> native f64 ------------------
+// real r = (spin*3+colour)*2+reim of site (tile, lane), slice s
+template <typename R>
+__device__ __forceinline__ size_t native_real_index(const Geom& g, int tile, int lane, int s, int r) {
+    constexpr int VW = (sizeof(R) == 8) ? 2 : 4;
+    constexpr int K = 24 / VW;
+    const int k = r / VW, j = r - k * VW;
+    return ((((size_t)tile * g.Ls + s) * K + k) * g.TS + lane) * VW + j;
+}
+
+// one thread per (native site, s).  canonical half field: [cb = lex/2][s][24]; FULL: [lex][s][24]
+template <typename R, bool UNPACK>
+__global__ void pack_kernel(Geom g, R* __restrict__ native, R* __restrict__ canon, int parity, int full) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (long long)g.Vh * g.Ls) return;
+    const int s = (int)(gid % g.Ls);
+    const int site = (int)(gid / g.Ls);
+    const int tile = site / g.TS, lane = site - tile * g.TS;
+    Coord c = site_coords(g, tile, lane, parity);
+    const long long lex = lex_index(g, c.x);
+    const long long csite = full ? lex : (lex >> 1);
+    R* cp = canon + (csite * g.Ls + s) * 24;
+#pragma unroll
+    for (int r = 0; r < 24; ++r) {
+        const size_t ni = native_real_index<R>(g, tile, lane, s, r);
+        if (UNPACK) cp[r] = native[ni]; else native[ni] = cp[r];
+    }
+}
+
+dwf_status launch_pack(dwf_ctx* c, void* native, const void* canon, int prec, int parity, bool unpack) {
+    const Geom& g = c->g;
+    const long long n = (long long)g.Vh * g.Ls;
+    const int block = 128;
+    const int grid = (int)((n + block - 1) / block);
+    const int p0 = (parity == DWF_FULL) ? 0 : parity, p1 = (parity == DWF_FULL) ? 1 : parity;
+    for (int par = p0; par <= p1; ++par) {
+        const size_t off = (parity == DWF_FULL && par == 1) ? half_bytes(g, prec) : 0;
+        void* nat = (char*)native + off;
+        const int full = (parity == DWF_FULL);
+        if (prec == DWF_F64) {
+            if (unpack) pack_kernel<double, true><<<grid, block, 0, c->stream>>>(g, (double*)nat, (double*)canon, par, full);
+            else pack_kernel<double, false><<<grid, block, 0, c->stream>>>(g, (double*)nat, (double*)canon, par, full);
+        } else {
+            if (unpack) pack_kernel<float, true><<<grid, block, 0, c->stream>>>(g, (float*)nat, (float*)canon, par, full);
+            else pack_kernel<float, false><<<grid, block, 0, c->stream>>>(g, (float*)nat, (float*)canon, par, full);
+        }
+        c->launches++;
+    }
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
+}
+
+// native -> native with a precision change; ACCUM: dst += src (used for x64 += e32)
+template <typename RD, typename RS, bool ACCUM>
+__global__ void convert_kernel(Geom g, RD* __restrict__ dst, const RS* __restrict__ src) {
+    // one thread per (tile, s, lane, group of 4 reals)
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long n = (long long)g.Vh * g.Ls * 6;
+    if (gid >= n) return;
+    const int lane = (int)(gid % g.TS);
+    long long r = gid / g.TS;
+    const int q = (int)(r % 6);
+    r /= 6;
+    const int s = (int)(r % g.Ls);
+    const int tile = (int)(r / g.Ls);
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+        const size_t si = native_real_index<RS>(g, tile, lane, s, q * 4 + j);
+        const size_t di = native_real_index<RD>(g, tile, lane, s, q * 4 + j);
+        if (ACCUM) dst[di] += (RD)src[si]; else dst[di] = (RD)src[si];
+    }
+}
+
+dwf_status launch_convert(dwf_ctx* c, void* dst, int dprec, const void* src, int sprec, size_t nhalf_fields) {
+    const Geom& g = c->g;
+    const long long n = (long long)g.Vh * g.Ls * 6;
+    const int block = 256;
+    const int grid = (int)((n + block - 1) / block);
+    for (size_t h = 0; h < nhalf_fields; ++h) {
+        void* d = (char*)dst + h * half_bytes(g, dprec);
+        const void* s = (const char*)src + h * half_bytes(g, sprec);
+        if (dprec == DWF_F32 && sprec == DWF_F64)
+            convert_kernel<float, double, false><<<grid, block, 0, c->stream>>>(g, (float*)d, (const double*)s);
+        else if (dprec == DWF_F64 && sprec == DWF_F32)
+            convert_kernel<double, float, false><<<grid, block, 0, c->stream>>>(g, (double*)d, (const float*)s);
+        else if (dprec == DWF_F64)
+            convert_kernel<double, double, false><<<grid, block, 0, c->stream>>>(g, (double*)d, (const double*)s);
+        else
+            convert_kernel<float, float, false><<<grid, block, 0, c->stream>>>(g, (float*)d, (const float*)s);
+        c->launches++;
+    }
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
+}
+
+dwf_status launch_add_f32_to_f64(dwf_ctx* c, void* x64, const void* e32, size_t) {
+    const Geom& g = c->g;
+    const long long n = (long long)g.Vh * g.Ls * 6;
+    const int block = 256;
+    const int grid = (int)((n + block - 1) / block);
+    convert_kernel<double, float, true><<<grid, block, 0, c->stream>>>(g, (double*)x64, (const float*)e32);
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
+}
+
+}  // namespace dwf

@@ -1,0 +1,118 @@
+// Internal declarations of the dwf_b200 library (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/dwf.h"
+
+namespace dwf {
+
+// ---------------------------------------------------------------------------------------------
+// Native layout.  One parity of a field:
+//     vec index = ((tile * Ls + s) * K + k) * TS + lane          (16-byte vectors)
+// K = 24/VW vectors per spinor (VW = 4 floats or 2 doubles), TS = sites of one parity in a tile.
+// tile = ((it*NT[2] + iz)*NT[1] + iy)*NT[0] + ix ; lane = ((tt*T[2] + tz)*T[1] + ty)*(T[0]/2) + tx/2.
+// Gauge, per OUTPUT parity: vec index = ((tile * 8 + leg) * KG + kg) * TS + lane, leg = 2*mu + dir,
+// dir 0: W = U_mu(x) (forward), dir 1: W = U_mu(x-mu)^dag (backward); 12 (rows 0,1) or 18 reals.
+// ---------------------------------------------------------------------------------------------
+struct Geom {
+    int L[4];    // lattice extents
+    int T[4];    // tile extents
+    int NT[4];   // tiles per direction
+    int TS;      // sites of one parity per tile
+    int ntiles;  // number of tiles
+    int Vh;      // sites of one parity  (= ntiles*TS)
+    int Ls;
+    int antiperiodic_t;
+};
+
+// 5-D coefficient tables: out_s = sum_s' Tp[s][s'] in_s' on P+ components (spin 0,1), Tm on P- (spin 2,3)
+struct Table5 {
+    double p[32 * 32];
+    double m[32 * 32];
+};
+
+enum Op5 { OP_A = 0, OP_ADAG, OP_MEE, OP_MEEDAG, OP_MEEINV, OP_MEEINVDAG,
+           OP_A_MEEINV,        // A * Mee^-1            (middle of Mpc)
+           OP_MEEINVDAG_ADAG,  // Mee^-dag * A^dag      (middle of Mpc^dag)
+           OP5_COUNT };
+
+struct DevTables {           // device copies, [OP5_COUNT][2][Ls*Ls]
+    double* d64 = nullptr;
+    float* d32 = nullptr;
+};
+
+}  // namespace dwf
+
+struct dwf_ctx {
+    dwf::Geom g;
+    double M5, mf, b5, c5;
+    int cut[4];
+    int compress12 = 1;
+    int tile_opt[4] = {0, 0, 0, 0};
+    int dhop_sc = 0;       // 0 = library default per precision
+    int dhop_loop_s = 0;
+    double inner_tol = 1e-4;
+    int max_restarts = 20;
+    cudaStream_t stream = nullptr;
+    bool gauge_set = false;
+    bool geom_frozen = false;
+    // gauge copies [parity]
+    void* W64[2] = {nullptr, nullptr};
+    void* W32[2] = {nullptr, nullptr};
+    size_t wbytes64 = 0, wbytes32 = 0;
+    dwf::Table5 tab[dwf::OP5_COUNT];
+    dwf::DevTables dtab;
+    // workspace (allocated lazily, sized for half fields)
+    void* ws64[10] = {};
+    void* ws32[10] = {};
+    double* partials = nullptr;  // per-block reduction partials
+    int npartials = 0;
+    double* scalars = nullptr;   // device scalars
+    double* scalars_host = nullptr;  // pinned
+    void* stage_dev[2] = {nullptr, nullptr};  // staging for *_host calls
+    size_t stage_bytes[2] = {0, 0};
+    long long launches = 0;
+    std::string err;
+};
+
+namespace dwf {
+
+inline size_t half_vecs(const Geom& g, int prec) { return (size_t)g.Vh * g.Ls * (prec == DWF_F64 ? 12 : 6); }
+inline size_t half_bytes(const Geom& g, int prec) { return half_vecs(g, prec) * 16; }
+
+#define DWF_CUDA_CHECK(ctx, expr)                                                            \
+    do {                                                                                     \
+        cudaError_t _e = (expr);                                                             \
+        if (_e != cudaSuccess) {                                                             \
+            (ctx)->err = std::string(#expr) + ": " + cudaGetErrorString(_e);                 \
+            return DWF_ECUDA;                                                                \
+        }                                                                                    \
+    } while (0)
+
+// kernels / launchers (one translation unit each)
+dwf_status launch_dhop(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec);
+// out = T[op1] x (+ yscale*y if y && op2<0 | + yscale*T[op2] y if y && op2>=0); norm_slot>=0: |out|^2 -> scalars[slot]
+dwf_status launch_op5(dwf_ctx* c, void* out, const void* x, int op1, const void* y, int op2, double yscale,
+                      int prec, int norm_slot);
+dwf_status launch_gauge_prep(dwf_ctx* c, const double* Ucanon);
+dwf_status launch_pack(dwf_ctx* c, void* native, const void* canon, int prec, int parity, bool unpack);
+dwf_status launch_convert(dwf_ctx* c, void* dst, int dprec, const void* src, int sprec, size_t nhalf_fields);
+// BLAS-1 on native half fields; scalar slots index c->scalars
+dwf_status launch_norm2(dwf_ctx* c, const void* v, int prec, size_t nreal, int slot);
+dwf_status launch_cg_update(dwf_ctx* c, void* x, void* r, const void* p, const void* z, int prec, size_t nreal,
+                            int slot_c, int slot_d, int slot_cn);            // x+=a p; r-=a z; cn=|r|^2, a=c/d
+dwf_status launch_xpay(dwf_ctx* c, void* p, const void* r, int prec, size_t nreal, int slot_cn, int slot_c);  // p=r+(cn/c)p
+dwf_status launch_axpy(dwf_ctx* c, void* y, const void* x, double a, int prec, size_t nreal);  // y += a x
+dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int prec, size_t nreal);  // out = a - b
+dwf_status launch_add_f32_to_f64(dwf_ctx* c, void* x64, const void* e32, size_t unused);  // x += (double)e, half field
+dwf_status ensure_partials(dwf_ctx* c, int n);
+dwf_status launch_reduce(dwf_ctx* c, int n, int slot);
+void build_tables(dwf_ctx* c);
+
+enum { SLOT_C = 0, SLOT_D, SLOT_CN, SLOT_B, SLOT_T0, SLOT_T1, NSLOTS = 16 };
+
+}  // namespace dwf
