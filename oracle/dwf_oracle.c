@@ -99,66 +99,85 @@ static inline long field_site(long lex, int parity_mode) {
     return parity_mode == 2 ? lex : lex / 2;
 }
 
+/* all Ls slices of one output site `lex`; osite = where the result goes in `out` */
+static void dhop_site(const orc_params* p, const cplx* Uc, const cplx* in, cplx* out, long lex, long osite,
+                      int out_parity, int dagger) {
+    const int Ls = p->Ls;
+    int x[4];
+    coords_of(p->L, lex, x);
+    for (int s = 0; s < Ls; ++s) {
+        cplx acc[4][3];
+        for (int a = 0; a < 4; ++a)
+            for (int c = 0; c < 3; ++c) acc[a][c] = 0;
+        for (int mu = 0; mu < 4; ++mu) {
+            for (int dir = 0; dir < 2; ++dir) { /* 0: forward leg, 1: backward leg */
+                int y[4] = {x[0], x[1], x[2], x[3]};
+                double bc = 1.0;
+                if (dir == 0) {
+                    y[mu] = (x[mu] + 1) % p->L[mu];
+                    if (mu == 3 && p->antiperiodic_t && x[3] == p->L[3] - 1) bc = -1.0;
+                } else {
+                    y[mu] = (x[mu] - 1 + p->L[mu]) % p->L[mu];
+                    if (mu == 3 && p->antiperiodic_t && x[3] == 0) bc = -1.0;
+                }
+                long ylex = lex_of(p->L, y);
+                const cplx* link = Uc + ((dir == 0 ? lex : ylex) * 4 + mu) * 9;
+                const cplx* psi = in + (field_site(ylex, out_parity) * Ls + s) * 12;
+                /* colour multiply: chi[a][c] = sum_c' W[c][c'] psi[a][c'] */
+                cplx chi[4][3];
+                for (int a = 0; a < 4; ++a)
+                    for (int c = 0; c < 3; ++c) {
+                        cplx t = 0;
+                        for (int cp = 0; cp < 3; ++cp) {
+                            cplx w = (dir == 0) ? link[c * 3 + cp] : conj(link[cp * 3 + c]);
+                            t += w * psi[a * 3 + cp];
+                        }
+                        chi[a][c] = (real)bc * t;
+                    }
+                /* spin: (1 -/+ gamma_mu), full 4x4 the slow way */
+                double sg = (dir == 0) ? -1.0 : +1.0;
+                if (dagger) sg = -sg;
+                for (int a = 0; a < 4; ++a)
+                    for (int c = 0; c < 3; ++c) {
+                        cplx t = chi[a][c];
+                        for (int b = 0; b < 4; ++b)
+                            t += (cplx)(sg * GAMMA[mu][a][b]) * chi[b][c];
+                        acc[a][c] += t;
+                    }
+            }
+        }
+        cplx* o = out + (osite * Ls + s) * 12;
+        for (int a = 0; a < 4; ++a)
+            for (int c = 0; c < 3; ++c) o[a * 3 + c] = acc[a][c];
+    }
+}
+
 void ORC(orc_dhop)(const orc_params* p, const real* U, const real* in_, real* out_,
                    int out_parity, int dagger) {
     const cplx* in = (const cplx*)in_;
     cplx* out = (cplx*)out_;
     const cplx* Uc = (const cplx*)U;
     const long V = vol4(p);
-    const int Ls = p->Ls;
 #pragma omp parallel for schedule(static)
     for (long lex = 0; lex < V; ++lex) {
         int x[4];
         coords_of(p->L, lex, x);
         int par = (x[0] + x[1] + x[2] + x[3]) & 1;
         if (out_parity != 2 && par != out_parity) continue;
-        long osite = field_site(lex, out_parity);
-        for (int s = 0; s < Ls; ++s) {
-            cplx acc[4][3];
-            for (int a = 0; a < 4; ++a)
-                for (int c = 0; c < 3; ++c) acc[a][c] = 0;
-            for (int mu = 0; mu < 4; ++mu) {
-                for (int dir = 0; dir < 2; ++dir) { /* 0: forward leg, 1: backward leg */
-                    int y[4] = {x[0], x[1], x[2], x[3]};
-                    double bc = 1.0;
-                    if (dir == 0) {
-                        y[mu] = (x[mu] + 1) % p->L[mu];
-                        if (mu == 3 && p->antiperiodic_t && x[3] == p->L[3] - 1) bc = -1.0;
-                    } else {
-                        y[mu] = (x[mu] - 1 + p->L[mu]) % p->L[mu];
-                        if (mu == 3 && p->antiperiodic_t && x[3] == 0) bc = -1.0;
-                    }
-                    long ylex = lex_of(p->L, y);
-                    const cplx* link = Uc + ((dir == 0 ? lex : ylex) * 4 + mu) * 9;
-                    const cplx* psi = in + (field_site(ylex, out_parity) * Ls + s) * 12;
-                    /* colour multiply: chi[a][c] = sum_c' W[c][c'] psi[a][c'] */
-                    cplx chi[4][3];
-                    for (int a = 0; a < 4; ++a)
-                        for (int c = 0; c < 3; ++c) {
-                            cplx t = 0;
-                            for (int cp = 0; cp < 3; ++cp) {
-                                cplx w = (dir == 0) ? link[c * 3 + cp] : conj(link[cp * 3 + c]);
-                                t += w * psi[a * 3 + cp];
-                            }
-                            chi[a][c] = (real)bc * t;
-                        }
-                    /* spin: (1 -/+ gamma_mu), full 4x4 the slow way */
-                    double sg = (dir == 0) ? -1.0 : +1.0;
-                    if (dagger) sg = -sg;
-                    for (int a = 0; a < 4; ++a)
-                        for (int c = 0; c < 3; ++c) {
-                            cplx t = chi[a][c];
-                            for (int b = 0; b < 4; ++b)
-                                t += (cplx)(sg * GAMMA[mu][a][b]) * chi[b][c];
-                            acc[a][c] += t;
-                        }
-                }
-            }
-            cplx* o = out + (osite * Ls + s) * 12;
-            for (int a = 0; a < 4; ++a)
-                for (int c = 0; c < 3; ++c) o[a * 3 + c] = acc[a][c];
-        }
+        dhop_site(p, Uc, in, out, lex, field_site(lex, out_parity), out_parity, dagger);
     }
+}
+
+/* The same per-site loop for a LIST of output sites (full-lattice lex indices, each of parity
+ * out_parity when out_parity != 2): out[i] = Dhop in at site lex_list[i], [i][s][spin][colour].
+ * Lets the tests check sampled outputs at sizes where a full oracle pass is slow.              */
+void ORC(orc_dhop_sites)(const orc_params* p, const real* U, const real* in_, real* out_, int out_parity,
+                         int dagger, long nsites, const long* lex_list) {
+    const cplx* in = (const cplx*)in_;
+    cplx* out = (cplx*)out_;
+    const cplx* Uc = (const cplx*)U;
+#pragma omp parallel for schedule(static)
+    for (long i = 0; i < nsites; ++i) dhop_site(p, Uc, in, out, lex_list[i], i, out_parity, dagger);
 }
 
 /* ---- C4: s-hop Q and its adjoint ---------------------------------------

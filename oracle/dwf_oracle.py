@@ -95,6 +95,16 @@ class Oracle:
                              int(out_parity), int(bool(dagger)))
         return out
 
+    def dhop_sites(self, psi, lex_list, out_parity=2, dagger=False):
+        """Dhop at the listed output sites only (full-lattice lex indices): [i, s, spin, colour]."""
+        psi = self._c(psi)
+        assert psi.shape == (self.full_shape() if out_parity == 2 else self.half_shape())
+        lex = np.ascontiguousarray(lex_list, dtype=np.int64)
+        out = np.empty((lex.size, self.Ls, 4, 3), dtype=self.cdtype)
+        self._fn("orc_dhop_sites")(ctypes.byref(self.p), self._ptr(self.U), self._ptr(psi), self._ptr(out),
+                                   int(out_parity), int(bool(dagger)), ctypes.c_long(lex.size), self._ptr(lex))
+        return out
+
     def _site_local(self, name, psi, dagger):
         psi = self._c(psi)
         n4 = psi.size // (self.Ls * 12)

@@ -1,0 +1,228 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same seeded inputs.  Bars (BASELINE.json north_star): fp64 operators 1e-12 relative L2, fp32 operators
+1e-5 relative L2 (fp64 oracle on the fp32-rounded inputs), CG true residual <= tol with the iteration
+count within +-2 of the oracle's."""
+import numpy as np
+import pytest
+
+from paper_2203_17119_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL = {"f64": 1e-12, "f32": 1e-5}
+MOEB = dict(M5=1.8, mf=0.01, b5=1.5, c5=0.5)
+SHAM = dict(M5=1.8, mf=0.1, b5=1.0, c5=0.0)
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.complex128)
+    b = np.asarray(b, dtype=np.complex128)
+    return float(np.linalg.norm((a - b).ravel()) / max(np.linalg.norm(b.ravel()), 1e-300))
+
+
+@pytest.fixture(scope="module")
+def api():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2203_17119_b200 import api as _api
+    _api.load_library()
+    return _api
+
+
+class Case:
+    """One lattice: gauge, GPU context(s), fp64 oracle (the fp32 GPU path is compared with the fp64 oracle
+    run on the fp32-rounded gauge and source, SURVEY §8(c) 'other silent points' (iii))."""
+
+    def __init__(self, api, dims, Ls, par, eps=0.4, cut=(0, 0, 0, 0), apbc=True, seed=7, compress12=1, tiles=None):
+        from oracle.dwf_oracle import Oracle
+        self.api, self.dims, self.Ls = api, tuple(dims), Ls
+        self.U = inputs.gauge_weak(dims, eps, seed)
+        opts = dict(antiperiodic_t=int(apbc), compress12=compress12)
+        if tiles:
+            opts.update({f"tile_{k}": v for k, v in zip("xyzt", tiles)})
+        self.gpu = api.Dwf(dims, Ls, par["M5"], par["mf"], par["b5"], par["c5"], cut=cut, **opts)
+        self.gpu.set_gauge(self.U)
+        self.orc = Oracle(dims, Ls, par["M5"], par["mf"], par["b5"], par["c5"], antiperiodic_t=apbc, cut=cut).set_gauge(self.U)
+        U32 = self.U.astype(np.complex64).astype(np.complex128)
+        self.orc_r32 = Oracle(dims, Ls, par["M5"], par["mf"], par["b5"], par["c5"], antiperiodic_t=apbc, cut=cut).set_gauge(U32)
+        self.full = inputs.source_full(dims, Ls, seed + 100)
+        self.even, self.odd = inputs.split_parity(self.full, dims)
+
+    def P(self, prec):
+        return self.api.F64 if prec == "f64" else self.api.F32
+
+    def src(self, a, prec):
+        return a if prec == "f64" else a.astype(np.complex64).astype(np.complex128)
+
+    def oracle(self, prec):
+        return self.orc if prec == "f64" else self.orc_r32
+
+    def full_native(self, prec):
+        g, P = self.gpu, self.P(prec)
+        import torch
+        return torch.cat([g.pack(self.even, P, self.api.EVEN), g.pack(self.odd, P, self.api.ODD)])
+
+    def unpack_full(self, nat, prec):
+        g, P = self.gpu, self.P(prec)
+        n = nat.numel() // 2
+        e = g.unpack(nat[:n], P, self.api.EVEN)
+        o = g.unpack(nat[n:], P, self.api.ODD)
+        return inputs.merge_parity(e, o, self.dims)
+
+
+CASES = {
+    # c1: BASELINE configs[0]
+    "c1": dict(dims=(4, 4, 4, 4), Ls=8, par=SHAM, eps=0.2),
+    # several tiles + a ragged mix of tile extents (6 -> tiles of 2), Moebius, Ls with a specialised kernel
+    "ragged": dict(dims=(8, 4, 6, 12), Ls=12, par=MOEB, eps=0.5),
+    # generic-Ls path (Ls = 5 has no unrolled instantiation), periodic t
+    "ls5": dict(dims=(4, 8, 4, 4), Ls=5, par=MOEB, eps=0.5, apbc=False),
+    # Dirichlet cut in t (c2's geometry scaled down) and a second cut in x
+    "cut": dict(dims=(8, 8, 8, 16), Ls=16, par=MOEB, eps=0.3, cut=(0, 0, 0, 8)),
+    "cut2": dict(dims=(8, 4, 4, 8), Ls=8, par=MOEB, eps=0.3, cut=(4, 0, 0, 4)),
+    # uncompressed 18-real links
+    "g18": dict(dims=(4, 4, 8, 8), Ls=8, par=MOEB, eps=0.7, compress12=0),
+    # smallest legal lattice, Ls = 1
+    "tiny": dict(dims=(2, 2, 2, 2), Ls=1, par=MOEB, eps=0.7),
+    # non-default tiles
+    "tiles": dict(dims=(8, 8, 4, 8), Ls=4, par=MOEB, eps=0.7, tiles=(8, 2, 2, 4)),
+}
+
+
+@pytest.fixture(scope="module", params=list(CASES))
+def case(request, api, oracle_built):
+    c = Case(api, **CASES[request.param])
+    yield c
+    c.gpu.close()
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_pack_unpack_roundtrip(case, prec):
+    g, P = case.gpu, case.P(prec)
+    src = case.src(case.odd, prec)
+    back = g.unpack(g.pack(src, P, case.api.ODD), P, case.api.ODD)
+    assert np.array_equal(back, src if prec == "f64" else src.astype(np.complex64))
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_dhop_half_and_full(case, prec, dagger):
+    g, P, A = case.gpu, case.P(prec), case.api
+    orc = case.oracle(prec)
+    e, o = case.src(case.even, prec), case.src(case.odd, prec)
+    out_e = g.unpack(g.dhop(g.pack(o, P, A.ODD), A.EVEN, dagger, P), P, A.EVEN)
+    out_o = g.unpack(g.dhop(g.pack(e, P, A.EVEN), A.ODD, dagger, P), P, A.ODD)
+    assert rel(out_e, orc.dhop(o, 0, dagger)) < TOL[prec]
+    assert rel(out_o, orc.dhop(e, 1, dagger)) < TOL[prec]
+    full = case.unpack_full(g.dhop(case.full_native(prec), A.FULL, dagger, P), prec)
+    assert rel(full, orc.dhop(case.src(case.full, prec), 2, dagger)) < TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dagger", [False, True])
+@pytest.mark.parametrize("op", ["meooe5d", "mooee", "mooee_inv"])
+def test_site_local_5d(case, prec, dagger, op):
+    g, P, A = case.gpu, case.P(prec), case.api
+    o = case.src(case.odd, prec)
+    got = g.unpack(getattr(g, op)(g.pack(o, P, A.ODD), A.ODD, dagger, P), P, A.ODD)
+    want = getattr(case.oracle(prec), op)(o, dagger)
+    assert rel(got, want) < TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+@pytest.mark.parametrize("dagger", [False, True])
+def test_M_full(case, prec, dagger):
+    g, P = case.gpu, case.P(prec)
+    got = case.unpack_full(g.m(case.full_native(prec), dagger, P), prec)
+    assert rel(got, case.oracle(prec).M(case.src(case.full, prec), dagger)) < TOL[prec]
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_mpc_mpcdag_mdagm(case, prec):
+    g, P, A = case.gpu, case.P(prec), case.api
+    orc = case.oracle(prec)
+    o = case.src(case.odd, prec)
+    nat = g.pack(o, P, A.ODD)
+    assert rel(g.unpack(g.mpc(nat, False, P), P, A.ODD), orc.mpc(o)) < TOL[prec]
+    assert rel(g.unpack(g.mpc(nat, True, P), P, A.ODD), orc.mpc(o, dagger=True)) < TOL[prec]
+    assert rel(g.unpack(g.mdagm(nat, P), P, A.ODD), orc.mdagm(o)) < 2 * TOL[prec]
+
+
+def test_norm2_and_convert(case):
+    g, A = case.gpu, case.api
+    nat = g.pack(case.odd, A.F64, A.ODD)
+    n = g.norm2(nat, A.F64, A.ODD)
+    assert abs(n - case.orc.norm2(case.odd)) <= 1e-13 * n
+    n32 = g.convert(nat, A.F64, A.F32, A.ODD)
+    back = g.unpack(n32, A.F32, A.ODD)
+    assert np.array_equal(back, case.odd.astype(np.complex64))
+    assert g.norm2(n32, A.F32, A.ODD) == pytest.approx(case.orc.norm2(case.odd.astype(np.complex64).astype(np.complex128)), rel=1e-12)
+
+
+def test_cg_f64_matches_oracle(case):
+    from oracle.dwf_oracle import cg
+    g, A = case.gpu, case.api
+    tol = 1e-10
+    x_ref, info_ref = cg(case.orc, case.odd, tol, 5000)
+    x, info, st = g.cg(g.pack(case.odd, A.F64, A.ODD), tol, 5000, A.CG_F64)
+    assert st == A.OK and info_ref["converged"]
+    assert info["resid_true"] <= tol
+    assert abs(info["iters_total"] - info_ref["iters"]) <= 2, (info, info_ref)
+    xs = g.unpack(x, A.F64, A.ODD)
+    # both solve to 1e-10 in the residual; the solutions agree to cond * tol
+    assert rel(xs, x_ref) < 1e-6
+    # the oracle recomputes the true residual of the GPU solution
+    r = case.odd - case.orc.mdagm(xs)
+    assert np.sqrt(case.orc.norm2(r) / case.orc.norm2(case.odd)) <= tol * (1 + 1e-6)
+
+
+def test_cg_mixed_matches_oracle(case):
+    from oracle.dwf_oracle import Oracle, cg_mixed
+    g, A = case.gpu, case.api
+    o64 = case.orc
+    o32 = Oracle(case.dims, case.Ls, o64.M5, o64.mf, o64.b5, o64.c5, antiperiodic_t=bool(o64.p.antiperiodic_t),
+                 cut=o64.cut, prec="f32").set_gauge(case.U)
+    tol = 1e-10
+    x_ref, info_ref = cg_mixed(o64, o32, case.odd, tol, 20000)
+    x, info, st = g.cg(g.pack(case.odd, A.F64, A.ODD), tol, 20000, A.CG_MIXED)
+    assert st == A.OK and info_ref["converged"]
+    assert info["resid_true"] <= tol
+    assert info["restarts"] == info_ref["restarts"], (info, info_ref)
+    # reading C9: +-2 per restart where fp32 rounding allows, else within 2 %
+    slack = max(2 * info_ref["restarts"], int(0.02 * info_ref["iters"]) + 1)
+    assert abs(info["iters_total"] - info_ref["iters"]) <= slack, (info, info_ref)
+    xs = g.unpack(x, A.F64, A.ODD)
+    r = case.odd - o64.mdagm(xs)
+    assert np.sqrt(o64.norm2(r) / o64.norm2(case.odd)) <= tol * (1 + 1e-6)
+
+
+def test_solve_full_system(case):
+    from oracle.dwf_oracle import solve_redblack
+    g, A = case.gpu, case.api
+    tol = 1e-10
+    psi_ref, info_ref = solve_redblack(case.orc, case.full, tol, 5000)
+    psi, info, st = g.solve(case.full_native("f64"), tol, 5000, A.CG_F64)
+    assert st == A.OK
+    got = case.unpack_full(psi, "f64")
+    assert abs(info["iters_total"] - info_ref["iters"]) <= 2
+    # the oracle applies M to the GPU solution
+    res = np.sqrt(case.orc.norm2(case.full - case.orc.M(got)) / case.orc.norm2(case.full))
+    assert res < 1e-7 and abs(info["resid_full"] - res) <= 1e-3 * res + 1e-13
+    assert rel(got, psi_ref) < 1e-6
+
+
+def test_host_entry_points(case):
+    """dwf_dhop_host / dwf_mdagm_host / dwf_solve_host: canonical HOST buffers in and out."""
+    g, A = case.gpu, case.api
+    src = np.ascontiguousarray(case.full)
+    out = np.empty_like(src)
+    g.dhop_host(out, src, A.FULL, False, A.F64)
+    assert rel(out, case.orc.dhop(case.full, 2, False)) < 1e-12
+    o = np.ascontiguousarray(case.odd)
+    out_o = np.empty_like(o)
+    g.mdagm_host(out_o, o, A.F64)
+    assert rel(out_o, case.orc.mdagm(case.odd)) < 2e-12
+    psi = np.empty_like(src)
+    _, info, st = g.solve_host(psi, src, 1e-9, 5000, A.CG_F64)
+    assert st == A.OK
+    assert np.sqrt(case.orc.norm2(case.full - case.orc.M(psi)) / case.orc.norm2(case.full)) < 1e-6
