@@ -1,0 +1,335 @@
+#!/usr/bin/env python
+"""bench.py — the hot path of arXiv:2203.17119 (Moebius DWF Dhop / Mpc^dag Mpc / red-black CG) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl dwf|reference] [--workload c4]
+
+One STEP = one pass of the whole hot path on one seeded synthetic subdomain (BASELINE.json configs[3]:
+32^4 x Ls=12 Moebius, the configuration the metric is quoted on): a fixed-length red-black CG segment
+`dwf_cg(max_iter = --cg-iters)` on Mpc^dag Mpc in fp64 -- every iteration is Mpc (A, Dhop_eo, A Mee^-1,
+Dhop_oe, Moo) + Mpc^dag + the fused axpy/norm kernels, plus the segment's |b|^2 and closing true residual.
+`value` is the step's nominal GFLOP/s (flop convention in DESIGN.md §6: 1320 per 5-D site per Dhop, 3000 per
+Mpc, 240 per iteration of BLAS-1), device-timed with inputs resident in HBM.  `e2e` is the same step through
+dwf_cg_host with pinned HOST buffers (H2D/D2H copies and layout packing inside the timed region).
+`roofline` is the dominant kernel (half-volume fp64 Dhop) timed per launch by CUDA events on the launching
+stream inside the timed steps.  Extra keys report the Dhop / Mpc^dag Mpc sweeps and CG time-to-solution.
+
+N > 1 (torchrun): the path shards by independent Dirichlet subdomains, one per rank, no
+data-path collective; timing is the max over ranks ("scaling": "weak").
+--impl reference: the CPU oracle (oracle/), as it stands, on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "DWF Dhop/Mpc^dag Mpc red-black CG hot-path throughput (1320 flop per 5-D site per Dhop)"
+UNIT = "GFLOP/s"
+FLOP_DHOP = 1320            # per 5-D output site
+FLOP_MPC = 2 * 1320 + 360   # per odd 5-D site (a5)
+FLOP_BLAS_ITER = 240        # x+=ap, r-=az, |r|^2, p=r+bp, |q|^2 : 5 x 48
+
+
+def segment_flops(n5h: int, iters: int) -> float:
+    """nominal flops of one CG segment on n5h odd 5-D sites: |b|^2, `iters` iterations, closing true residual."""
+    per_iter = 2 * FLOP_MPC + FLOP_BLAS_ITER
+    closing = 2 * FLOP_MPC + 24 + 48      # A x, b - Ax, |.|^2
+    return float(n5h) * (48 + iters * per_iter + closing)
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        self.t.join(timeout=2)
+        sm, smax, reasons = [], [], set()
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); smax.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def make_inputs(cfg, rank: int):
+    from paper_2203_17119_b200 import inputs
+    import dataclasses
+    c = dataclasses.replace(cfg, gauge_seed=cfg.gauge_seed + 100 * rank, source_seed=cfg.source_seed + 100 * rank)
+    U = inputs.make_gauge(c)
+    b = inputs.source_half(c.dims, c.Ls, c.source_seed, parity=1)
+    return U, b
+
+
+# ------------------------------------------------------------------------------------------- reference arm
+def oracle_segment(sample_dims, cfg, iters, steps, warmup):
+    """The oracle's CG (oracle/dwf_oracle.py cg, as it stands) for `iters` iterations on a sample lattice."""
+    from oracle.dwf_oracle import Oracle, cg
+    from paper_2203_17119_b200 import inputs
+    U = inputs.gauge_weak(sample_dims, cfg.eps, cfg.gauge_seed)
+    b = inputs.source_half(sample_dims, cfg.Ls, cfg.source_seed, parity=1)
+    orc = Oracle(sample_dims, cfg.Ls, cfg.M5, cfg.mf, cfg.b5, cfg.c5, antiperiodic_t=cfg.antiperiodic_t,
+                 cut=cfg.cut).set_gauge(U)
+    n5h = b.shape[0] * cfg.Ls
+    for _ in range(warmup):
+        cg(orc, b, 1e-300, iters)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        cg(orc, b, 1e-300, iters)
+    dt = (time.perf_counter() - t0) / max(steps, 1)
+    return segment_flops(n5h, iters) / dt / 1e9, dt, n5h
+
+
+def run_reference(args, cfg):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    sample = tuple(args.ref_dims)
+    cores = os.cpu_count()
+    val, dt, n5h = oracle_segment(sample, cfg, args.ref_iters, args.steps, args.warmup)
+    desc = (f"oracle CG segment ({args.ref_iters} iteration(s) + closing true residual) on a "
+            f"{'x'.join(map(str, sample))} x Ls={cfg.Ls} sample of {cfg.name} (same parameters, seeds and recipe)")
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "sample": desc},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def workload_name(cfg):
+    return (f"{cfg.name}: {'x'.join(map(str, cfg.dims))} x Ls={cfg.Ls} Moebius b5={cfg.b5} c5={cfg.c5} M5={cfg.M5} "
+            f"mf={cfg.mf}, gauge exp(i*{cfg.eps}*H) seeded SU(3), 2-row compressed links (BASELINE.json configs[3])")
+
+
+# ------------------------------------------------------------------------------------------------ own arm
+def ev_time(torch, fn, reps):
+    s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    s.record()
+    for _ in range(reps):
+        fn()
+    e.record()
+    torch.cuda.synchronize()
+    return s.elapsed_time(e) / reps
+
+
+def run_dwf(args, cfg):
+    import torch
+    import torch.distributed as dist
+    from paper_2203_17119_b200 import api
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the hot path has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    hbm_peak, peak_src = peaks()
+
+    U, b_np = make_inputs(cfg, rank)
+    g = api.from_config(cfg, device=f"cuda:{local}")
+    g.set_gauge(U)
+    del U
+    A = api
+    b = g.pack(b_np, A.F64, A.ODD)
+    x = g.new_native(A.F64, A.ODD)
+    n5h = (cfg.V4 // 2) * cfg.Ls
+    iters = args.cg_iters
+
+    def step():
+        g.cg(b, 1e-300, iters, A.CG_F64, x=x, use_guess=False)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    # ---- timed region: K steps, device-timed, per-launch Dhop events on the ctx stream
+    sampler = ClockSampler(local)
+    sampler.start()
+    g.set_option("time_dhop", 1)
+    l0 = g.launch_count()
+    barrier()
+    s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    s.record()
+    for _ in range(args.steps):
+        step()
+    e.record()
+    barrier()
+    ms = s.elapsed_time(e)
+    dhop_ms, dhop_n = g.get_option("dhop_ms"), g.get_option("dhop_timed")
+    launches = g.launch_count() - l0
+    g.set_option("time_dhop", 0)
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    ms_step = ms / args.steps
+    value = world * segment_flops(n5h, iters) / (ms_step * 1e-3) / 1e9
+
+    # ---- roofline of the dominant kernel: half-volume fp64 Dhop
+    ng = 12
+    dhop_bytes = n5h * 48 * 8 + (cfg.V4 // 2) * 8 * ng * 8
+    dhop_avg_ms = dhop_ms / max(dhop_n, 1)
+    achieved = dhop_bytes / (dhop_avg_ms * 1e-3) / 1e9
+    traffic = None
+    tp = os.path.join(ROOT, "profiles", "dhop_traffic.json")
+    if os.path.exists(tp):
+        traffic = json.load(open(tp)).get("dhop_f64_dram_bytes_per_launch")
+    roofline = {"bound": "hbm", "kernel": "dhop_kernel<double> (half-volume, 12-real links)", "achieved": achieved,
+                "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / hbm_peak,
+                "traffic": traffic, "algorithmic_bytes_per_launch": dhop_bytes, "avg_launch_ms": dhop_avg_ms,
+                "launches_timed": int(dhop_n), "share_of_step": dhop_ms / ms if ms > 0 else None,
+                "gflops": FLOP_DHOP * n5h / (dhop_avg_ms * 1e-3) / 1e9}
+
+    # ---- e2e: the same step through the C ABI with pinned HOST buffers
+    b_host = torch.from_numpy(np.ascontiguousarray(b_np).view(np.float64).reshape(-1)).pin_memory()
+    x_host = torch.empty_like(b_host).pin_memory()
+    g.cg_host(x_host, b_host, 1e-300, iters)
+    barrier()
+    t0 = time.perf_counter()
+    e2e_steps = max(1, min(args.steps, 5))
+    for _ in range(e2e_steps):
+        g.cg_host(x_host, b_host, 1e-300, iters)
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+    if world > 1:
+        t = torch.tensor([e2e_s], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    hb = b_host.numel() * 8
+    e2e = {"value": world * segment_flops(n5h, iters) / e2e_s / 1e9, "unit": UNIT, "h2d_bytes_per_step": hb,
+           "d2h_bytes_per_step": hb, "ms_per_step": e2e_s * 1e3, "call": "dwf_cg_host (pinned canonical fp64 buffers)"}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "impl": "dwf",
+            "config": {"workload": workload_name(cfg), "step": f"dwf_cg fp64 segment: {iters} iterations + |b|^2 + closing true residual",
+                       "l2": "inputs_larger_than_L2 (each half field 1.2 GB, gauge 0.4 GB per parity)", "parallelism": f"independent subdomains x{world}"},
+            "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "e2e": e2e}
+
+    if rank == 0 and not args.no_extras:
+        line["sweeps"] = sweeps(torch, g, A, cfg, hbm_peak)
+        line["cg"] = cg_solutions(g, A, b, cfg, args)
+    if rank == 0 and world == 1 and not args.no_cpu:
+        sample = tuple(args.ref_dims)
+        val, dt, _ = oracle_segment(sample, cfg, args.ref_iters, 2, 1)
+        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "s_per_step": dt,
+                                "sample": f"oracle CG segment ({args.ref_iters} iteration(s) + closing true residual) on a "
+                                          f"{'x'.join(map(str, sample))} x Ls={cfg.Ls} sample of {cfg.name}, 2 timed repetitions"}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
+def sweeps(torch, g, A, cfg, hbm_peak):
+    """Kernel-alone sweeps (CUDA events, 3 warm-ups): full-volume Dhop and Mpc^dag Mpc in fp32 and fp64."""
+    out = {}
+    n5h = (cfg.V4 // 2) * cfg.Ls
+    for prec, name, B in ((A.F32, "f32", 4), (A.F64, "f64", 8)):
+        src = g.new_native(prec, A.FULL).normal_()
+        dst = g.new_native(prec, A.FULL)
+        for _ in range(3):
+            g.dhop(src, A.FULL, False, prec, out=dst)
+        ms = ev_time(torch, lambda: g.dhop(src, A.FULL, False, prec, out=dst), 20)
+        by = 2 * (n5h * 48 * B + (cfg.V4 // 2) * 8 * 12 * B)
+        out[f"dhop_{name}"] = {"ms_full_volume": ms, "gflops": FLOP_DHOP * 2 * n5h / ms / 1e6, "gbs": by / ms / 1e6,
+                               "frac_hbm": by / ms / 1e6 / hbm_peak}
+        so, do = src[: src.numel() // 2], dst[: dst.numel() // 2]
+        for _ in range(3):
+            g.mdagm(so, prec, out=do)
+        ms = ev_time(torch, lambda: g.mdagm(so, prec, out=do), 10)
+        by = 2 * (5 * n5h * 24 * B + 2 * (cfg.V4 // 2) * 8 * 12 * B)      # fused minimum 5 S_h + 2 G_h per Mpc
+        out[f"mdagm_{name}"] = {"ms": ms, "gflops": 2 * FLOP_MPC * n5h / ms / 1e6, "gbs_fused_minimum": by / ms / 1e6,
+                                "frac_hbm_fused_minimum": by / ms / 1e6 / hbm_peak}
+        del src, dst
+    return out
+
+
+def cg_solutions(g, A, b, cfg, args):
+    """red-black CG time-to-solution on the workload (fp64 and fp32-inner/fp64-outer), once each."""
+    out = {}
+    for mode, name in ((A.CG_F64, "f64"), (A.CG_MIXED, "mixed")):
+        x, info, st = g.cg(b, cfg.tol, args.max_iter, mode)
+        out[name] = {"tol": cfg.tol, "status": int(st), "iters": info["iters_total"], "restarts": info["restarts"],
+                     "resid_true": info["resid_true"], "time_to_solution_s": info["seconds"], "launches": info["launches"]}
+        del x
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="dwf", choices=["dwf", "reference"])
+    ap.add_argument("--workload", default="c4")
+    ap.add_argument("--cg-iters", type=int, default=10)
+    ap.add_argument("--max-iter", type=int, default=20000)
+    ap.add_argument("--ref-dims", type=int, nargs=4, default=[16, 16, 16, 16])
+    ap.add_argument("--ref-iters", type=int, default=1)
+    ap.add_argument("--no-extras", action="store_true", help="skip the kernel sweeps and CG time-to-solution")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    from paper_2203_17119_b200 import inputs
+    cfg = inputs.CONFIGS[args.workload]
+    if args.impl == "reference":
+        run_reference(args, cfg)
+    else:
+        run_dwf(args, cfg)
+
+
+if __name__ == "__main__":
+    main()

@@ -76,7 +76,10 @@ dwf_status dwf_destroy(dwf_ctx* ctx);
  *   "antiperiodic_t" 0/1 (default 1)       "compress12" 0/1 (default 1; 2-row links, reading C10)
  *   "tile_x","tile_y","tile_z","tile_t"    native tile extents (default 4, or 2 where 4 does not divide)
  *   "inner_tol" (default 1e-4), "max_restarts" (default 20)     mixed-precision CG (reading C9), any time
- *   "dhop_sc" s-slices per thread in the Dhop kernel, "dhop_loop_s" 0/1, any time (tuning) */
+ *   "dhop_sc" s-slices per thread in the Dhop kernel, "dhop_loop_s" 0/1, any time (tuning)
+ *   "time_dhop" 0/1: bracket every Dhop kernel launch with CUDA events on the context stream (restarts the
+ *   accumulators); dwf_get_option "dhop_ms" / "dhop_timed" then synchronise and return the summed kernel time
+ *   and the number of launches timed (bench.py's roofline figure) */
 dwf_status dwf_set_option(dwf_ctx* ctx, const char* key, double val);
 dwf_status dwf_get_option(const dwf_ctx* ctx, const char* key, double* val);
 /* cudaStream_t as void* (torch.cuda.current_stream().cuda_stream); NULL = default stream */
@@ -130,6 +133,9 @@ dwf_status dwf_dhop_host(dwf_ctx* ctx, void* out_host, const void* in_host, dwf_
                          dwf_prec prec);
 /* out_host = Mpc^dag Mpc in_host; canonical ODD fields */
 dwf_status dwf_mdagm_host(dwf_ctx* ctx, void* out_host, const void* in_host, dwf_prec prec);
+/* x_host = (Mpc^dag Mpc)^-1 b_host from x = 0; canonical ODD fp64 fields; same stopping rule as dwf_cg */
+dwf_status dwf_cg_host(dwf_ctx* ctx, void* x_host, const void* b_host, double tol, int max_iter, dwf_cg_mode mode,
+                       dwf_cg_info* info);
 /* psi_host = M^-1 eta_host; canonical FULL fp64 fields */
 dwf_status dwf_solve_host(dwf_ctx* ctx, void* psi_host, const void* eta_host, double tol, int max_iter,
                           dwf_cg_mode mode, dwf_cg_info* info);

@@ -28,7 +28,7 @@ SYMBOLS = [
     "dwf_create", "dwf_destroy", "dwf_set_option", "dwf_get_option", "dwf_set_stream", "dwf_set_gauge",
     "dwf_field_bytes", "dwf_pack", "dwf_unpack", "dwf_convert", "dwf_dhop", "dwf_meooe5d", "dwf_mooee",
     "dwf_mooee_inv", "dwf_m", "dwf_mpc", "dwf_mdagm", "dwf_norm2", "dwf_cg", "dwf_solve", "dwf_dhop_host",
-    "dwf_mdagm_host", "dwf_solve_host", "dwf_launch_count", "dwf_last_error", "dwf_version",
+    "dwf_mdagm_host", "dwf_cg_host", "dwf_solve_host", "dwf_launch_count", "dwf_last_error", "dwf_version",
 ]
 
 
@@ -84,6 +84,7 @@ def load_library():
     lib.dwf_dhop_host.argtypes = [vp, vp, vp, ci, ci, ci]
     lib.dwf_mdagm_host.argtypes = [vp, vp, vp, ci]
     lib.dwf_solve_host.argtypes = [vp, vp, vp, cd, ci, ci, P(CgInfo)]
+    lib.dwf_cg_host.argtypes = [vp, vp, vp, cd, ci, ci, P(CgInfo)]
     lib.dwf_launch_count.argtypes = [vp]
     lib.dwf_launch_count.restype = ctypes.c_longlong
     lib.dwf_last_error.argtypes = [vp]
@@ -248,9 +249,10 @@ class Dwf:
         return r.value
 
     # ---- solvers ---------------------------------------------------------------------------------
-    def cg(self, b, tol, max_iter, mode=CG_F64, x=None):
-        """Mpc^dag Mpc x = b on native fp64 ODD fields.  Returns (x, info dict, status)."""
-        use_guess = x is not None
+    def cg(self, b, tol, max_iter, mode=CG_F64, x=None, use_guess=None):
+        """Mpc^dag Mpc x = b on native fp64 ODD fields.  Returns (x, info dict, status).
+        x given: it is the output buffer and, unless use_guess=False, the initial guess."""
+        use_guess = (x is not None) if use_guess is None else bool(use_guess)
         x = self.new_native(F64, ODD) if x is None else x
         info = CgInfo()
         st = self._chk(self.lib.dwf_cg(self._h, self._p(x), self._p(b), tol, max_iter, mode, int(use_guess),
@@ -281,6 +283,12 @@ class Dwf:
     def mdagm_host(self, out_host, in_host, prec=F64):
         self._chk(self.lib.dwf_mdagm_host(self._h, self._hp(out_host), self._hp(in_host), prec))
         return out_host
+
+    def cg_host(self, x_host, b_host, tol, max_iter, mode=CG_F64):
+        info = CgInfo()
+        st = self._chk(self.lib.dwf_cg_host(self._h, self._hp(x_host), self._hp(b_host), tol, max_iter, mode,
+                                            ctypes.byref(info)), allow=(ENOTCONV,))
+        return x_host, info.as_dict(), st
 
     def solve_host(self, psi_host, eta_host, tol, max_iter, mode=CG_F64):
         info = CgInfo()

@@ -328,6 +328,8 @@ dwf_status dwf_destroy(dwf_ctx* c) {
         if (c->ws64[i]) cudaFree(c->ws64[i]);
         if (c->ws32[i]) cudaFree(c->ws32[i]);
     }
+    for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
+    pipe_tables_free(c);
     if (c->partials) cudaFree(c->partials);
     if (c->scalars) cudaFree(c->scalars);
     if (c->scalars_host) cudaFreeHost(c->scalars_host);
@@ -357,6 +359,14 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
     else if (k == "max_restarts") c->max_restarts = (int)val;
     else if (k == "dhop_sc") { if (val < 0 || val > 4) return DWF_EINVAL; c->dhop_sc = (int)val; }
     else if (k == "dhop_loop_s") c->dhop_loop_s = (val != 0.0);
+    else if (k == "dhop_kernel") c->dhop_kernel = (int)val;
+    else if (k == "dhop_nst") { if (val != 2 && val != 3) return DWF_EINVAL; c->dhop_nst = (int)val; }
+    else if (k == "time_dhop") {       // (re)start per-launch event timing of the Dhop kernel
+        DWF_TRY(dhop_timing_flush(c));
+        c->time_dhop = (val != 0.0);
+        c->dhop_ms = 0.0;
+        c->dhop_timed = 0;
+    }
     else { c->err = "unknown option '" + k + "'"; return DWF_EINVAL; }
     return DWF_OK;
 }
@@ -364,6 +374,12 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
 dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
     if (!c || !key || !val) return DWF_EINVAL;
     const std::string k(key);
+    if (k == "dhop_ms" || k == "dhop_timed") {   // synchronises: folds the pending event pairs
+        dwf_ctx* m = const_cast<dwf_ctx*>(c);
+        DWF_TRY(dhop_timing_flush(m));
+        *val = (k == "dhop_ms") ? m->dhop_ms : (double)m->dhop_timed;
+        return DWF_OK;
+    }
     if (k == "antiperiodic_t") *val = c->g.antiperiodic_t;
     else if (k == "compress12") *val = c->compress12;
     else if (k == "tile_x") *val = c->g.T[0];
@@ -374,6 +390,9 @@ dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
     else if (k == "max_restarts") *val = c->max_restarts;
     else if (k == "dhop_sc") *val = c->dhop_sc;
     else if (k == "dhop_loop_s") *val = c->dhop_loop_s;
+    else if (k == "time_dhop") *val = c->time_dhop;
+    else if (k == "dhop_kernel") *val = c->dhop_kernel;
+    else if (k == "dhop_nst") *val = c->dhop_nst;
     else return DWF_EINVAL;
     return DWF_OK;
 }
@@ -398,6 +417,7 @@ dwf_status dwf_set_gauge(dwf_ctx* c, const void* U) {
     c->wbytes64 = b64;
     c->wbytes32 = b32;
     DWF_TRY(launch_gauge_prep(c, (const double*)U));
+    DWF_TRY(pipe_tables_upload(c));
     c->gauge_set = true;
     return DWF_OK;
 }
@@ -582,6 +602,29 @@ dwf_status dwf_mdagm_host(dwf_ctx* c, void* out_host, const void* in_host, dwf_p
     DWF_CUDA_CHECK(c, cudaMemcpyAsync(out_host, canon, nb, cudaMemcpyDeviceToHost, c->stream));
     DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
     return DWF_OK;
+}
+
+dwf_status dwf_cg_host(dwf_ctx* c, void* x_host, const void* b_host, double tol, int max_iter, dwf_cg_mode mode,
+                       dwf_cg_info* info) {
+    DWF_TRY(need_gauge(c));
+    if (!x_host || !b_host) return DWF_EINVAL;
+    const double t0 = now_s();
+    const long long l0 = c->launches;
+    const size_t nb = dwf_field_bytes(c, DWF_F64, DWF_ODD);
+    void *canon, *nat;
+    DWF_TRY(stage_get(c, 0, nb, &canon));
+    DWF_TRY(stage_get(c, 1, 2 * nb, &nat));
+    void* nat_b = nat;
+    void* nat_x = (char*)nat + nb;
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(canon, b_host, nb, cudaMemcpyHostToDevice, c->stream));
+    DWF_TRY(launch_pack(c, nat_b, canon, DWF_F64, DWF_ODD, false));
+    dwf_status st = dwf_cg(c, nat_x, nat_b, tol, max_iter, mode, 0, info);
+    if (st != DWF_OK && st != DWF_ENOTCONV) return st;
+    DWF_TRY(launch_pack(c, nat_x, canon, DWF_F64, DWF_ODD, true));
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(x_host, canon, nb, cudaMemcpyDeviceToHost, c->stream));
+    DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (info) { info->seconds = now_s() - t0; info->launches = (int)(c->launches - l0); }
+    return st;
 }
 
 dwf_status dwf_solve_host(dwf_ctx* c, void* psi_host, const void* eta_host, double tol, int max_iter, dwf_cg_mode mode,

@@ -55,6 +55,13 @@ struct dwf_ctx {
     int tile_opt[4] = {0, 0, 0, 0};
     int dhop_sc = 0;       // 0 = library default per precision
     int dhop_loop_s = 0;
+    int dhop_kernel = 0;   // 0 = auto (pipelined tile kernel when the tile shape has one), 1 = generic kernel
+    int dhop_nst = 3;      // ring depth of the pipelined fp32 kernel
+    // tables of the pipelined Dhop kernel (dwf_dhop_pipe.cu), built at dwf_set_gauge
+    uint16_t* pipe_nbslot = nullptr;
+    int16_t* pipe_slot_dir = nullptr;
+    uint16_t* pipe_slot_lane = nullptr;
+    int pipe_nslot = 0;
     double inner_tol = 1e-4;
     int max_restarts = 20;
     cudaStream_t stream = nullptr;
@@ -76,6 +83,12 @@ struct dwf_ctx {
     void* stage_dev[2] = {nullptr, nullptr};  // staging for *_host calls
     size_t stage_bytes[2] = {0, 0};
     long long launches = 0;
+    // optional per-launch CUDA-event timing of the Dhop kernel ("time_dhop" option; bench.py's roofline)
+    int time_dhop = 0;
+    std::vector<cudaEvent_t> ev;     // pairs (start, stop)
+    int ev_used = 0;
+    double dhop_ms = 0.0;
+    long long dhop_timed = 0;
     std::string err;
 };
 
@@ -112,6 +125,10 @@ dwf_status launch_add_f32_to_f64(dwf_ctx* c, void* x64, const void* e32, size_t 
 dwf_status ensure_partials(dwf_ctx* c, int n);
 dwf_status launch_reduce(dwf_ctx* c, int n, int slot);
 void build_tables(dwf_ctx* c);
+dwf_status pipe_tables_upload(dwf_ctx* c);
+void pipe_tables_free(dwf_ctx* c);
+dwf_status launch_dhop_pipe(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, bool* handled);
+dwf_status dhop_timing_flush(dwf_ctx* c);   // synchronises the stream, folds recorded event pairs into dhop_ms
 
 enum { SLOT_C = 0, SLOT_D, SLOT_CN, SLOT_B, SLOT_T0, SLOT_T1, NSLOTS = 16 };
 
