@@ -330,6 +330,7 @@ dwf_status dwf_destroy(dwf_ctx* c) {
     }
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     pipe_tables_free(c);
+    tma_state_free(c);
     if (c->partials) cudaFree(c->partials);
     if (c->scalars) cudaFree(c->scalars);
     if (c->scalars_host) cudaFreeHost(c->scalars_host);
@@ -360,6 +361,7 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
     else if (k == "dhop_sc") { if (val < 0 || val > 4) return DWF_EINVAL; c->dhop_sc = (int)val; }
     else if (k == "dhop_loop_s") c->dhop_loop_s = (val != 0.0);
     else if (k == "dhop_kernel") c->dhop_kernel = (int)val;
+    else if (k == "dhop_grid") { if (val < 0) return DWF_EINVAL; c->dhop_grid = (int)val; }
     else if (k == "dhop_nst") { if (val != 2 && val != 3) return DWF_EINVAL; c->dhop_nst = (int)val; }
     else if (k == "time_dhop") {       // (re)start per-launch event timing of the Dhop kernel
         DWF_TRY(dhop_timing_flush(c));
@@ -393,6 +395,7 @@ dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
     else if (k == "time_dhop") *val = c->time_dhop;
     else if (k == "dhop_kernel") *val = c->dhop_kernel;
     else if (k == "dhop_nst") *val = c->dhop_nst;
+    else if (k == "dhop_grid") *val = c->dhop_grid;
     else return DWF_EINVAL;
     return DWF_OK;
 }
@@ -418,6 +421,7 @@ dwf_status dwf_set_gauge(dwf_ctx* c, const void* U) {
     c->wbytes32 = b32;
     DWF_TRY(launch_gauge_prep(c, (const double*)U));
     DWF_TRY(pipe_tables_upload(c));
+    DWF_TRY(tma_state_build(c));
     c->gauge_set = true;
     return DWF_OK;
 }

@@ -166,6 +166,11 @@ dwf_status launch_dhop(dwf_ctx* c, void* out, const void* in, int out_parity, in
 }
 
 static dwf_status launch_dhop_untimed(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec) {
+    if (c->dhop_kernel == 0) {
+        bool handled = false;
+        dwf_status st = launch_dhop_tma(c, out, in, out_parity, dagger, prec, &handled);
+        if (st != DWF_OK || handled) return st;
+    }
     if (c->dhop_kernel != 1) {
         bool handled = false;
         dwf_status st = launch_dhop_pipe(c, out, in, out_parity, dagger, prec, &handled);

@@ -1,0 +1,555 @@
+// Dhop, warp-specialised TMA kernel for 4x4x4x4 tiles (the fast path on sm_100a).
+//
+// Persistent CTAs walk the tiles in an L2-friendly sweep order.  Per CTA:
+//   * warp group 0 is the PRODUCER (one warp active, registers shrunk with setmaxnreg): for every
+//     (tile, s) it fills one stage of an NST-deep shared-memory ring with the s-slice working set of
+//     the tile -- 12 regions of [K][32 slots] 16-byte vectors:
+//        regions 0-3   the tile's own four t-slabs           (TMA, 512-byte rows)
+//        regions 4,5   +t / -t faces of the neighbour tiles  (TMA, 512-byte rows)
+//        regions 6,7   +z / -z faces                         (TMA, 128-byte rows)
+//        regions 8,9   +y / -y faces                         (TMA, 32-byte rows)
+//        regions 10,11 +x / -x faces                         (cp.async gather: the checkerboard makes the x
+//                                                             face a row-parity pattern no box can describe)
+//     ten cp.async.bulk.tensor boxes + 2K cp.async per lane, all completing on the stage's `full`
+//     mbarrier; the next tile's links are prefetched into L2 with one bulk prefetch;
+//   * the other warp groups are CONSUMERS: each thread keeps its links in registers for the whole s
+//     loop (third row rebuilt once per tile, antiperiodic sign folded in), waits on `full`, reads its
+//     neighbours with 128-bit LDS at a uniform 512-byte k pitch, spin-projects, multiplies,
+//     reconstruct-accumulates, releases the stage on the `empty` mbarrier and stores 128-bit
+//     coalesced with a streaming hint.  No block-wide barrier inside the loop: warps drift apart and
+//     keep the FP and shared-memory pipes busy at the same time.
+// fp32: one thread per site (8 links in registers), 2 CTAs/SM.  fp64: two lanes (l, l^16) per site (forward legs
+// on one, backward legs on the other), partial sums exchanged by warp shuffles, 1 CTA/SM.
+#include <cuda.h>
+
+#include <algorithm>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+#include "dwf_dhop_math.cuh"
+
+namespace dwf {
+
+// ------------------------------------------------------------------------------------------ host tables
+namespace {
+
+constexpr int TSV = 128;      // sites of one parity in a 4^4 tile
+constexpr int NREG = 12;      // regions per stage
+
+struct TmaTables {
+    std::vector<uint16_t> off;     // [2][8][128]  stage offset (16-byte units, k = 0) of the leg's neighbour
+    std::vector<uint8_t> xsrc;     // [2][2][32]   source lane (in the +x / -x tile) of each x-face slot
+};
+
+inline int lane_of(int tx, int ty, int tz, int tt) { return ((tt * 4 + tz) * 4 + ty) * 2 + (tx >> 1); }
+
+TmaTables build_tma_tables(int K) {
+    TmaTables t;
+    t.off.assign(2 * 8 * TSV, 0);
+    t.xsrc.assign(2 * 2 * 32, 0);
+    for (int p = 0; p < 2; ++p) {
+        const int q = 1 - p;   // input parity
+        for (int tt = 0; tt < 4; ++tt)
+            for (int tz = 0; tz < 4; ++tz)
+                for (int ty = 0; ty < 4; ++ty) {
+                    const int row = (tt * 4 + tz) * 4 + ty;
+                    // x-face slots: row >> 1 enumerates the rows of the needed parity (ty alternates inside (tz,tt))
+                    if (((q + ty + tz + tt) & 1) == 0) t.xsrc[(p * 2 + 0) * 32 + (row >> 1)] = (uint8_t)(row * 2 + 0);   // +x tile, tx = 0
+                    else                               t.xsrc[(p * 2 + 1) * 32 + (row >> 1)] = (uint8_t)(row * 2 + 1);   // -x tile, tx = 3
+                    for (int txh = 0; txh < 2; ++txh) {
+                        const int tx = 2 * txh + ((p + ty + tz + tt) & 1);
+                        const int lane = lane_of(tx, ty, tz, tt);
+                        for (int leg = 0; leg < 8; ++leg) {
+                            const int mu = leg >> 1;
+                            int y[4] = {tx, ty, tz, tt};
+                            y[mu] += (leg & 1) ? -1 : +1;
+                            int region, slot;
+                            if (y[mu] >= 0 && y[mu] < 4) {
+                                region = y[3];
+                                slot = (y[2] * 4 + y[1]) * 2 + (y[0] >> 1);
+                            } else {
+                                const int up = (y[mu] >= 4);
+                                y[mu] = (y[mu] + 4) & 3;
+                                const int yh = y[0] >> 1;
+                                if (mu == 3)      { region = up ? 4 : 5;   slot = (y[2] * 4 + y[1]) * 2 + yh; }
+                                else if (mu == 2) { region = up ? 6 : 7;   slot = y[3] * 8 + y[1] * 2 + yh; }
+                                else if (mu == 1) { region = up ? 8 : 9;   slot = (y[3] * 4 + y[2]) * 2 + yh; }
+                                else              { region = up ? 10 : 11; slot = ((y[3] * 4 + y[2]) * 4 + y[1]) >> 1; }
+                            }
+                            t.off[(p * 8 + leg) * TSV + lane] = (uint16_t)(region * K * 32 + slot);
+                        }
+                    }
+                }
+    }
+    return t;
+}
+
+// Tile traversal: sweep t with an (x: all, y: all, z: pairs) cross-section, so that the tiles in flight plus the
+// ones just done form a slab whose +-x, +-y, -t and one z neighbour are in L2.
+std::vector<uint32_t> build_order(const Geom& g) {
+    std::vector<uint32_t> o;
+    o.reserve(g.ntiles);
+    const int zb = (g.NT[2] % 2 == 0) ? 2 : 1;
+    for (int z0 = 0; z0 < g.NT[2]; z0 += zb)
+        for (int t = 0; t < g.NT[3]; ++t)
+            for (int z = z0; z < z0 + zb; ++z)
+                for (int y = 0; y < g.NT[1]; ++y)
+                    for (int x = 0; x < g.NT[0]; ++x) {
+                        const int c[4] = {x, y, z, t};
+                        o.push_back((uint32_t)tile_index(g, c));
+                    }
+    return o;
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                  const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                  CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qres) == cudaSuccess &&
+            qres == cudaDriverEntryPointSuccess)
+            fn = (EncodeTiledFn)p;
+        cudaGetLastError();
+    }
+    return fn;
+}
+
+}  // namespace
+
+struct TmaState {
+    uint16_t* off = nullptr;      // device [2][8][128]
+    uint8_t* xsrc = nullptr;      // device [2][2][32]
+    uint32_t* order = nullptr;    // device [ntiles]
+    int K_built = 0;
+    int num_sms = 0;
+    struct Maps { const void* ptr; int prec; CUtensorMap m[3]; };
+    std::vector<Maps> cache;      // small LRU of tensor maps per input pointer
+};
+
+void tma_state_free(dwf_ctx* c) {
+    TmaState* s = (TmaState*)c->tma;
+    if (!s) return;
+    if (s->off) cudaFree(s->off);
+    if (s->xsrc) cudaFree(s->xsrc);
+    if (s->order) cudaFree(s->order);
+    delete s;
+    c->tma = nullptr;
+}
+
+// built at dwf_set_gauge (geometry is frozen there); returns DWF_OK with c->tma == nullptr when the tile shape
+// or the driver has no TMA path
+dwf_status tma_state_build(dwf_ctx* c) {
+    tma_state_free(c);
+    const Geom& g = c->g;
+    for (int mu = 0; mu < 4; ++mu)
+        if (g.T[mu] != 4) return DWF_OK;
+    if (!encode_fn()) return DWF_OK;
+    TmaState* s = new TmaState();
+    c->tma = s;
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    // offsets depend on K: fp64 table first, fp32 second
+    TmaTables t64 = build_tma_tables(12), t32 = build_tma_tables(6);
+    std::vector<uint16_t> off(t64.off);
+    off.insert(off.end(), t32.off.begin(), t32.off.end());
+    std::vector<uint32_t> order = build_order(g);
+    DWF_CUDA_CHECK(c, cudaMalloc(&s->off, off.size() * sizeof(uint16_t)));
+    DWF_CUDA_CHECK(c, cudaMalloc(&s->xsrc, t64.xsrc.size()));
+    DWF_CUDA_CHECK(c, cudaMalloc(&s->order, order.size() * sizeof(uint32_t)));
+    DWF_CUDA_CHECK(c, cudaMemcpy(s->off, off.data(), off.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+    DWF_CUDA_CHECK(c, cudaMemcpy(s->xsrc, t64.xsrc.data(), t64.xsrc.size(), cudaMemcpyHostToDevice));
+    DWF_CUDA_CHECK(c, cudaMemcpy(s->order, order.data(), order.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    return DWF_OK;
+}
+
+// three tensor maps over one native half field: [0] t-slabs (512-byte rows), [1] z faces (128-byte rows),
+// [2] y faces (32-byte rows).  A native half field is nrows = ntiles*Ls*K rows of 2048 bytes (one (tile,s,k) each).
+static dwf_status get_maps(dwf_ctx* c, const void* in, int prec, const CUtensorMap** out) {
+    TmaState* s = (TmaState*)c->tma;
+    for (size_t i = 0; i < s->cache.size(); ++i)
+        if (s->cache[i].ptr == in && s->cache[i].prec == prec) {
+            if (i != 0) std::swap(s->cache[i], s->cache[0]);
+            *out = s->cache[0].m;
+            return DWF_OK;
+        }
+    const Geom& g = c->g;
+    const int K = (prec == DWF_F64) ? 12 : 6;
+    const int epv = (prec == DWF_F64) ? 2 : 4;             // elements per 16-byte vector
+    const cuuint64_t nrows = (cuuint64_t)g.ntiles * g.Ls * K;
+    const CUtensorMapDataType dt = (prec == DWF_F64) ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
+    TmaState::Maps m;
+    m.ptr = in; m.prec = prec;
+    EncodeTiledFn enc = encode_fn();
+    const cuuint32_t ones[4] = {1, 1, 1, 1};
+    CUresult r;
+    {   // slabs: (32 lanes, tt, row)
+        const cuuint64_t dims[3] = {(cuuint64_t)32 * epv, 4, nrows};
+        const cuuint64_t strides[2] = {512, 2048};
+        const cuuint32_t box[3] = {(cuuint32_t)32 * epv, 1, (cuuint32_t)K};
+        r = enc(&m.m[0], dt, 3, const_cast<void*>(in), dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { c->err = "cuTensorMapEncodeTiled(slab) failed"; return DWF_ECUDA; }
+    }
+    {   // z faces: (8 lanes = ty,txh; tz; tt; row)
+        const cuuint64_t dims[4] = {(cuuint64_t)8 * epv, 4, 4, nrows};
+        const cuuint64_t strides[3] = {128, 512, 2048};
+        const cuuint32_t box[4] = {(cuuint32_t)8 * epv, 1, 4, (cuuint32_t)K};
+        r = enc(&m.m[1], dt, 4, const_cast<void*>(in), dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { c->err = "cuTensorMapEncodeTiled(z) failed"; return DWF_ECUDA; }
+    }
+    {   // y faces: (2 lanes = txh; ty; (tz,tt); row)
+        const cuuint64_t dims[4] = {(cuuint64_t)2 * epv, 4, 16, nrows};
+        const cuuint64_t strides[3] = {32, 128, 2048};
+        const cuuint32_t box[4] = {(cuuint32_t)2 * epv, 1, 16, (cuuint32_t)K};
+        r = enc(&m.m[2], dt, 4, const_cast<void*>(in), dims, strides, box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+        if (r != CUDA_SUCCESS) { c->err = "cuTensorMapEncodeTiled(y) failed"; return DWF_ECUDA; }
+    }
+    s->cache.insert(s->cache.begin(), m);
+    if (s->cache.size() > 32) s->cache.pop_back();
+    *out = s->cache[0].m;
+    return DWF_OK;
+}
+
+// ------------------------------------------------------------------------------------------ device helpers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    do {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void cp_async16_tma(uint32_t dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_mbar_arrive_noinc(uint32_t bar) {
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
+                 ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, uint32_t bar) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
+                 ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+
+__device__ __forceinline__ float4 lds_v(const float4*, uint32_t a) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double2 lds_v(const double2*, uint32_t a) {
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void stcs_v(float4* p, const float4& v) { __stcs(p, v); }
+__device__ __forceinline__ void stcs_v(double2* p, const double2& v) { __stcs(p, v); }
+
+__device__ __forceinline__ float shfl16(float v) { return __shfl_xor_sync(0xffffffffu, v, 16); }
+__device__ __forceinline__ double shfl16(double v) { return __shfl_xor_sync(0xffffffffu, v, 16); }
+
+// h = upper two rows of (1 + s*gamma_MU) psi, s = +-1 at run time (FMA form)
+template <typename R, int MU>
+__device__ __forceinline__ void proj_s(const R (&psi)[24], R s, R (&h)[12]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int p0 = 2 * c, p1 = 6 + 2 * c, p2 = 12 + 2 * c, p3 = 18 + 2 * c;
+        const int h0 = 2 * c, h1 = 6 + 2 * c;
+        if (MU == 0) {
+            h[h0] = psi[p0] - s * psi[p3 + 1]; h[h0 + 1] = psi[p0 + 1] + s * psi[p3];
+            h[h1] = psi[p1] - s * psi[p2 + 1]; h[h1 + 1] = psi[p1 + 1] + s * psi[p2];
+        } else if (MU == 1) {
+            h[h0] = psi[p0] - s * psi[p3]; h[h0 + 1] = psi[p0 + 1] - s * psi[p3 + 1];
+            h[h1] = psi[p1] + s * psi[p2]; h[h1 + 1] = psi[p1 + 1] + s * psi[p2 + 1];
+        } else if (MU == 2) {
+            h[h0] = psi[p0] - s * psi[p2 + 1]; h[h0 + 1] = psi[p0 + 1] + s * psi[p2];
+            h[h1] = psi[p1] + s * psi[p3 + 1]; h[h1 + 1] = psi[p1 + 1] - s * psi[p3];
+        } else {
+            h[h0] = psi[p0] + s * psi[p2]; h[h0 + 1] = psi[p0 + 1] + s * psi[p2 + 1];
+            h[h1] = psi[p1] + s * psi[p3]; h[h1 + 1] = psi[p1 + 1] + s * psi[p3 + 1];
+        }
+    }
+}
+
+// acc (+)= reconstruct((1 + s*gamma_MU) from g); FIRST: assign instead of accumulate
+template <typename R, int MU, bool FIRST>
+__device__ __forceinline__ void recon_s(const R (&g)[12], R s, R (&acc)[24]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int g0 = 2 * c, g1 = 6 + 2 * c;
+        const int a0 = 2 * c, a1 = 6 + 2 * c, a2 = 12 + 2 * c, a3 = 18 + 2 * c;
+        R l2r, l2i, l3r, l3i;   // lower rows
+        if (MU == 0)      { l2r = s * g[g1 + 1]; l2i = -s * g[g1]; l3r = s * g[g0 + 1]; l3i = -s * g[g0]; }
+        else if (MU == 1) { l2r = s * g[g1]; l2i = s * g[g1 + 1]; l3r = -s * g[g0]; l3i = -s * g[g0 + 1]; }
+        else if (MU == 2) { l2r = s * g[g0 + 1]; l2i = -s * g[g0]; l3r = -s * g[g1 + 1]; l3i = s * g[g1]; }
+        else              { l2r = s * g[g0]; l2i = s * g[g0 + 1]; l3r = s * g[g1]; l3i = s * g[g1 + 1]; }
+        if (FIRST) {
+            acc[a0] = g[g0]; acc[a0 + 1] = g[g0 + 1]; acc[a1] = g[g1]; acc[a1 + 1] = g[g1 + 1];
+            acc[a2] = l2r; acc[a2 + 1] = l2i; acc[a3] = l3r; acc[a3 + 1] = l3i;
+        } else {
+            acc[a0] += g[g0]; acc[a0 + 1] += g[g0 + 1]; acc[a1] += g[g1]; acc[a1 + 1] += g[g1 + 1];
+            if (MU == 0)      { acc[a2] += s * g[g1 + 1]; acc[a2 + 1] -= s * g[g1]; acc[a3] += s * g[g0 + 1]; acc[a3 + 1] -= s * g[g0]; }
+            else if (MU == 1) { acc[a2] += s * g[g1]; acc[a2 + 1] += s * g[g1 + 1]; acc[a3] -= s * g[g0]; acc[a3 + 1] -= s * g[g0 + 1]; }
+            else if (MU == 2) { acc[a2] += s * g[g0 + 1]; acc[a2 + 1] -= s * g[g0]; acc[a3] -= s * g[g1 + 1]; acc[a3 + 1] += s * g[g1]; }
+            else              { acc[a2] += s * g[g0]; acc[a2 + 1] += s * g[g0 + 1]; acc[a3] += s * g[g1]; acc[a3 + 1] += s * g[g1 + 1]; }
+        }
+    }
+}
+
+struct TmaArgs {
+    Geom g;
+    const void* in;
+    void* out;
+    const void* W;
+    const uint16_t* off;      // [8][128]   (this output parity, this precision)
+    const uint8_t* xsrc;      // [2][32]    (this output parity)
+    const uint32_t* order;    // [ntiles]
+    int dagger;
+};
+
+template <typename R, int TPS, int NG, int NST, int MINB>
+__global__ void __launch_bounds__(128 + 128 * TPS, MINB)
+dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, const __grid_constant__ CUtensorMap map_z,
+                const __grid_constant__ CUtensorMap map_y) {
+    using V = typename VT<R>::V;
+    constexpr int K = VT<R>::K, VW = VT<R>::VW;
+    constexpr int KG = (NG + VW - 1) / VW;
+    constexpr int LPT = 8 / TPS;
+    constexpr int NCW = 4 * TPS;                       // consumer warps
+    constexpr uint32_t REGION_BYTES = K * 512;
+    constexpr uint32_t STAGE_BYTES = NREG * REGION_BYTES;
+    constexpr int REG_PROD = 24;
+    constexpr int REG_CONS = (TPS == 2) ? 240 : 232;
+
+    extern __shared__ __align__(1024) unsigned char smem_raw[];
+    __shared__ __align__(8) unsigned long long bars[2 * NST];   // full[NST], empty[NST]
+
+    const Geom& g = a.g;
+    const int Ls = g.Ls;
+    const int tid = threadIdx.x;
+    const int warp = tid >> 5, lane = tid & 31;
+    const uint32_t stage0 = smem_u32(smem_raw);
+    const uint32_t bar0 = smem_u32(bars);
+    const int ntiles = g.ntiles;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int i = 0; i < NST; ++i) {
+            mbar_init(bar0 + 8 * i, 1 + 32);             // full: producer's expect_tx arrive + 32 cp.async arrivals
+            mbar_init(bar0 + 8 * (NST + i), NCW);        // empty: one arrival per consumer warp
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp < 4) {
+        // ================================================================================== PRODUCER
+        reg_dec<REG_PROD>();
+        if (warp != 0) return;
+        const V* __restrict__ in = reinterpret_cast<const V*>(a.in);
+        const unsigned xs_p = a.xsrc[lane], xs_m = a.xsrc[32 + lane];
+        const uint32_t tile_vecs = (uint32_t)Ls * K * TSV;
+        uint32_t n = 0;
+        for (int it = blockIdx.x; it < ntiles; it += gridDim.x) {
+            const int tile = a.order[it];
+            int tc[4];
+            tile_coords(g, tile, tc);
+            int nt[8];
+#pragma unroll
+            for (int mu = 0; mu < 4; ++mu) {
+                int nc[4] = {tc[0], tc[1], tc[2], tc[3]};
+                nc[mu] = (tc[mu] + 1 == g.NT[mu]) ? 0 : tc[mu] + 1;
+                nt[2 * mu] = tile_index(g, nc);
+                nc[mu] = (tc[mu] == 0) ? g.NT[mu] - 1 : tc[mu] - 1;
+                nt[2 * mu + 1] = tile_index(g, nc);
+            }
+            if (lane == 0 && it + (int)gridDim.x < ntiles) {     // next tile's links -> L2
+                const int nx = a.order[it + gridDim.x];
+                l2_prefetch_bulk(reinterpret_cast<const V*>(a.W) + (size_t)nx * 8 * KG * TSV, 8 * KG * TSV * 16);
+            }
+            const V* src_p = in + (size_t)nt[0] * tile_vecs + xs_p;
+            const V* src_m = in + (size_t)nt[1] * tile_vecs + xs_m;
+            for (int s = 0; s < Ls; ++s, ++n) {
+                const uint32_t st = n % NST, ph = (n / NST) & 1;
+                const uint32_t full = bar0 + 8 * st, empty = bar0 + 8 * (NST + st);
+                const uint32_t base = stage0 + st * STAGE_BYTES;
+                mbar_wait(empty, ph ^ 1);
+                if (lane == 0) {
+                    mbar_arrive_expect_tx(full, 10 * REGION_BYTES);
+                    const int row_own = (tile * Ls + s) * K;
+#pragma unroll
+                    for (int tt = 0; tt < 4; ++tt) tma_load_3d(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full);
+                    tma_load_3d(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full);
+                    tma_load_3d(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full);
+                    tma_load_4d(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full);
+                    tma_load_4d(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full);
+                    tma_load_4d(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full);
+                    tma_load_4d(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full);
+                }
+                const V* sp = src_p + (size_t)s * (K * TSV);
+                const V* sm = src_m + (size_t)s * (K * TSV);
+                const uint32_t dp = base + 10 * REGION_BYTES + lane * 16, dm = base + 11 * REGION_BYTES + lane * 16;
+#pragma unroll
+                for (int k = 0; k < K; ++k) {
+                    cp_async16_tma(dp + k * 512, sp + k * TSV);
+                    cp_async16_tma(dm + k * 512, sm + k * TSV);
+                }
+                cp_async_mbar_arrive_noinc(full);
+            }
+        }
+        return;
+    }
+
+    // ====================================================================================== CONSUMERS
+    reg_inc<REG_CONS>();
+    const int ctid = tid - 128;
+    const int cw = ctid >> 5;
+    int sub, site;
+    if (TPS == 1) { sub = 0; site = ctid; }
+    else { sub = lane >> 4; site = cw * 16 + (lane & 15); }
+
+    uint32_t myoff[LPT];
+#pragma unroll
+    for (int j = 0; j < LPT; ++j) {
+        const int leg = (TPS == 1) ? j : 2 * j + sub;
+        myoff[j] = (uint32_t)a.off[leg * TSV + site] * 16u;
+    }
+    const int tt = site >> 5;
+    const R dsgn = a.dagger ? (R)-1 : (R)1;
+    uint32_t n = 0;
+    for (int it = blockIdx.x; it < ntiles; it += gridDim.x) {
+        const int tile = a.order[it];
+        const int tct = tile / (g.NT[0] * g.NT[1] * g.NT[2]);
+        const int tglob = tct * 4 + tt;
+        // ---- links to registers (once per tile): rows 0,1 (+ row 2 rebuilt), antiperiodic sign folded in
+        R u[LPT][18];
+        {
+            const V* __restrict__ Wt = reinterpret_cast<const V*>(a.W) + (size_t)tile * 8 * KG * TSV + site;
+#pragma unroll
+            for (int j = 0; j < LPT; ++j) {
+                const int leg = (TPS == 1) ? j : 2 * j + sub;
+                load_link<R, NG>(Wt + (size_t)leg * KG * TSV, TSV, u[j]);
+                const int mu = (TPS == 1) ? (j >> 1) : j;
+                if (mu == 3 && g.antiperiodic_t) {
+                    const int dir = (TPS == 1) ? (j & 1) : sub;
+                    const bool flip = dir ? (tglob == 0) : (tglob == g.L[3] - 1);
+                    if (flip) {
+#pragma unroll
+                        for (int i = 0; i < 18; ++i) u[j][i] = -u[j][i];
+                    }
+                }
+            }
+        }
+        V* __restrict__ outp = reinterpret_cast<V*>(a.out) + (size_t)tile * Ls * K * TSV + site;
+        for (int s = 0; s < Ls; ++s, ++n) {
+            const uint32_t st = n % NST, ph = (n / NST) & 1;
+            const uint32_t base = stage0 + st * STAGE_BYTES;
+            mbar_wait(bar0 + 8 * st, ph);
+            R acc[24];
+#pragma unroll
+            for (int j = 0; j < LPT; ++j) {
+                const int mu = (TPS == 1) ? (j >> 1) : j;
+                const int dir = (TPS == 1) ? (j & 1) : sub;
+                const R sg = (dir ? (R)1 : (R)-1) * dsgn;     // forward leg: (1 - gamma), backward: (1 + gamma)
+                R psi[24], h[12], gg[12];
+                const uint32_t p = base + myoff[j];
+#pragma unroll
+                for (int k = 0; k < K; ++k) unpackv(lds_v((const V*)nullptr, p + k * 512), psi + k * VW);
+                if (j == 0) { proj_s<R, 0>(psi, sg, h); su3_mul<R>(u[j], h, gg); recon_s<R, 0, true>(gg, sg, acc); }
+                else if (mu == 0) { proj_s<R, 0>(psi, sg, h); su3_mul<R>(u[j], h, gg); recon_s<R, 0, false>(gg, sg, acc); }
+                else if (mu == 1) { proj_s<R, 1>(psi, sg, h); su3_mul<R>(u[j], h, gg); recon_s<R, 1, false>(gg, sg, acc); }
+                else if (mu == 2) { proj_s<R, 2>(psi, sg, h); su3_mul<R>(u[j], h, gg); recon_s<R, 2, false>(gg, sg, acc); }
+                else { proj_s<R, 3>(psi, sg, h); su3_mul<R>(u[j], h, gg); recon_s<R, 3, false>(gg, sg, acc); }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar0 + 8 * (NST + st));      // stage released
+            V* o = outp + (size_t)s * (K * TSV);
+            if (TPS == 1) {
+#pragma unroll
+                for (int k = 0; k < K; ++k) stcs_v(o + k * TSV, packv(acc + k * VW));
+            } else {
+                // lane pair (l, l^16): each keeps one chirality half of the 24 sums, sends the other
+                R mine[12];
+#pragma unroll
+                for (int i = 0; i < 12; ++i) {
+                    const R send = sub ? acc[i] : acc[12 + i];
+                    const R keep = sub ? acc[12 + i] : acc[i];
+                    mine[i] = keep + shfl16(send);
+                }
+                V* o2 = o + (sub ? (K / 2) * TSV : 0);
+#pragma unroll
+                for (int k = 0; k < K / 2; ++k) stcs_v(o2 + k * TSV, packv(mine + k * VW));
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------ launch
+template <typename R, int TPS, int NG, int NST, int MINB>
+static dwf_status launch_tma_t(dwf_ctx* c, const TmaArgs& a, const CUtensorMap* maps) {
+    constexpr int K = VT<R>::K;
+    const size_t smem = (size_t)NST * NREG * K * 512;
+    auto kern = dhop_tma_kernel<R, TPS, NG, NST, MINB>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        DWF_CUDA_CHECK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        attr_done = true;
+    }
+    TmaState* s = (TmaState*)c->tma;
+    int grid = s->num_sms * MINB;
+    if (c->dhop_grid > 0) grid = c->dhop_grid;
+    if (grid > c->g.ntiles) grid = c->g.ntiles;
+    kern<<<grid, 128 + 128 * TPS, smem, c->stream>>>(a, maps[0], maps[1], maps[2]);
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
+}
+
+dwf_status launch_dhop_tma(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, bool* handled) {
+    *handled = false;
+    TmaState* s = (TmaState*)c->tma;
+    if (!s) return DWF_OK;
+    const CUtensorMap* maps = nullptr;
+    dwf_status st = get_maps(c, in, prec, &maps);
+    if (st != DWF_OK) return st;
+    TmaArgs a;
+    a.g = c->g; a.in = in; a.out = out;
+    a.W = (prec == DWF_F64) ? c->W64[out_parity] : c->W32[out_parity];
+    a.off = s->off + (size_t)(prec == DWF_F64 ? 0 : 2 * 8 * TSV) + (size_t)out_parity * 8 * TSV;
+    a.xsrc = s->xsrc + (size_t)out_parity * 2 * 32;
+    a.order = s->order;
+    a.dagger = dagger;
+    *handled = true;
+    if (prec == DWF_F64)
+        return c->compress12 ? launch_tma_t<double, 2, 12, 3, 1>(c, a, maps) : launch_tma_t<double, 2, 18, 3, 1>(c, a, maps);
+    return c->compress12 ? launch_tma_t<float, 1, 12, 3, 2>(c, a, maps) : launch_tma_t<float, 1, 18, 3, 2>(c, a, maps);
+}
+
+}  // namespace dwf

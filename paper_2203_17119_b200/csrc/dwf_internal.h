@@ -55,8 +55,10 @@ struct dwf_ctx {
     int tile_opt[4] = {0, 0, 0, 0};
     int dhop_sc = 0;       // 0 = library default per precision
     int dhop_loop_s = 0;
-    int dhop_kernel = 0;   // 0 = auto (pipelined tile kernel when the tile shape has one), 1 = generic kernel
+    int dhop_kernel = 0;   // 0 = auto (TMA kernel for 4^4 tiles, else cp.async tile kernel, else generic), 1 = generic, 2 = cp.async tile kernel
     int dhop_nst = 3;      // ring depth of the pipelined fp32 kernel
+    int dhop_grid = 0;     // CTAs of the persistent TMA kernel (0 = SMs x resident CTAs)
+    void* tma = nullptr;   // dwf::TmaState (dwf_dhop_tma.cu), built at dwf_set_gauge for 4^4 tiles
     // tables of the pipelined Dhop kernel (dwf_dhop_pipe.cu), built at dwf_set_gauge
     uint16_t* pipe_nbslot = nullptr;
     int16_t* pipe_slot_dir = nullptr;
@@ -128,6 +130,9 @@ void build_tables(dwf_ctx* c);
 dwf_status pipe_tables_upload(dwf_ctx* c);
 void pipe_tables_free(dwf_ctx* c);
 dwf_status launch_dhop_pipe(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, bool* handled);
+dwf_status tma_state_build(dwf_ctx* c);
+void tma_state_free(dwf_ctx* c);
+dwf_status launch_dhop_tma(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, bool* handled);
 dwf_status dhop_timing_flush(dwf_ctx* c);   // synchronises the stream, folds recorded event pairs into dhop_ms
 
 enum { SLOT_C = 0, SLOT_D, SLOT_CN, SLOT_B, SLOT_T0, SLOT_T1, NSLOTS = 16 };
