@@ -362,6 +362,11 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
     else if (k == "dhop_loop_s") c->dhop_loop_s = (val != 0.0);
     else if (k == "dhop_kernel") c->dhop_kernel = (int)val;
     else if (k == "dhop_grid") { if (val < 0) return DWF_EINVAL; c->dhop_grid = (int)val; }
+    else if (k == "dhop_order" || k == "dhop_order_axes") {
+        if (val < 0 || val > 9999) return DWF_EINVAL;
+        (k == "dhop_order" ? c->dhop_order : c->dhop_order_axes) = (int)val;
+        if (c->gauge_set) DWF_TRY(tma_state_build(c));
+    }
     else if (k == "dhop_nst") { if (val != 2 && val != 3) return DWF_EINVAL; c->dhop_nst = (int)val; }
     else if (k == "time_dhop") {       // (re)start per-launch event timing of the Dhop kernel
         DWF_TRY(dhop_timing_flush(c));
@@ -396,6 +401,8 @@ dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
     else if (k == "dhop_kernel") *val = c->dhop_kernel;
     else if (k == "dhop_nst") *val = c->dhop_nst;
     else if (k == "dhop_grid") *val = c->dhop_grid;
+    else if (k == "dhop_order") *val = c->dhop_order;
+    else if (k == "dhop_order_axes") *val = c->dhop_order_axes;
     else return DWF_EINVAL;
     return DWF_OK;
 }

@@ -85,20 +85,50 @@ TmaTables build_tma_tables(int K) {
     return t;
 }
 
-// Tile traversal: sweep t with an (x: all, y: all, z: pairs) cross-section, so that the tiles in flight plus the
-// ones just done form a slab whose +-x, +-y, -t and one z neighbour are in L2.
-std::vector<uint32_t> build_order(const Geom& g) {
+// Tile traversal.  The persistent CTAs take order[blockIdx], order[blockIdx + grid], ...: at any time the tiles in
+// flight are about one grid-sized run of `order`.  The runs are compact 4-D blobs of B[0] x B[1] x B[2] x B[3] tiles
+// (faces between tiles of one blob are read by two CTAs at about the same time: L2 hits), and the blobs follow each
+// other in a boustrophedon path (axes[0] fastest), so that a blob's faces towards the previous blob are still in L2.
+// code = B0 B1 B2 B3 as decimal digits (0 = full extent), axes = fastest-first axis digits of the blob path
+// (DESIGN.md §5).  Default: 8x8x2x1 blobs swept along t, then z.
+std::vector<uint32_t> build_order(const Geom& g, int code, int axes_code) {
+    int B[4], ax[4];
+    if (code <= 0) { code = 21; axes_code = 3210; }   // 0 0 2 1
+    int digs[4] = {(code / 1000) % 10, (code / 100) % 10, (code / 10) % 10, code % 10};
+    for (int mu = 0; mu < 4; ++mu) {
+        B[mu] = digs[mu] <= 0 ? g.NT[mu] : std::min(digs[mu], g.NT[mu]);
+        while (g.NT[mu] % B[mu] != 0) --B[mu];
+    }
+    int ad[4] = {(axes_code / 1000) % 10, (axes_code / 100) % 10, (axes_code / 10) % 10, axes_code % 10};
+    bool seen[4] = {false, false, false, false};
+    int na = 0;
+    for (int i = 0; i < 4; ++i)
+        if (ad[i] >= 0 && ad[i] < 4 && !seen[ad[i]]) { ax[na++] = ad[i]; seen[ad[i]] = true; }
+    for (int mu = 3; mu >= 0; --mu)
+        if (!seen[mu]) { ax[na++] = mu; seen[mu] = true; }
+    int NB[4];
+    for (int mu = 0; mu < 4; ++mu) NB[mu] = g.NT[mu] / B[mu];
     std::vector<uint32_t> o;
     o.reserve(g.ntiles);
-    const int zb = (g.NT[2] % 2 == 0) ? 2 : 1;
-    for (int z0 = 0; z0 < g.NT[2]; z0 += zb)
-        for (int t = 0; t < g.NT[3]; ++t)
-            for (int z = z0; z < z0 + zb; ++z)
-                for (int y = 0; y < g.NT[1]; ++y)
-                    for (int x = 0; x < g.NT[0]; ++x) {
-                        const int c[4] = {x, y, z, t};
+    const int nblobs = NB[0] * NB[1] * NB[2] * NB[3];
+    for (int ib = 0; ib < nblobs; ++ib) {
+        // mixed-radix digits of ib (ax[0] fastest), reflected when the sum of the higher digits is odd
+        int d[4], r = ib;
+        for (int i = 0; i < 4; ++i) { d[i] = r % NB[ax[i]]; r /= NB[ax[i]]; }
+        int bc[4];
+        for (int i = 3; i >= 0; --i) {
+            int hi = 0;
+            for (int j = i + 1; j < 4; ++j) hi += d[j];
+            bc[ax[i]] = (hi & 1) ? NB[ax[i]] - 1 - d[i] : d[i];
+        }
+        for (int t = 0; t < B[3]; ++t)
+            for (int z = 0; z < B[2]; ++z)
+                for (int y = 0; y < B[1]; ++y)
+                    for (int x = 0; x < B[0]; ++x) {
+                        const int c[4] = {bc[0] * B[0] + x, bc[1] * B[1] + y, bc[2] * B[2] + z, bc[3] * B[3] + t};
                         o.push_back((uint32_t)tile_index(g, c));
                     }
+    }
     return o;
 }
 
@@ -160,7 +190,7 @@ dwf_status tma_state_build(dwf_ctx* c) {
     TmaTables t64 = build_tma_tables(12), t32 = build_tma_tables(6);
     std::vector<uint16_t> off(t64.off);
     off.insert(off.end(), t32.off.begin(), t32.off.end());
-    std::vector<uint32_t> order = build_order(g);
+    std::vector<uint32_t> order = build_order(g, c->dhop_order, c->dhop_order_axes);
     DWF_CUDA_CHECK(c, cudaMalloc(&s->off, off.size() * sizeof(uint16_t)));
     DWF_CUDA_CHECK(c, cudaMalloc(&s->xsrc, t64.xsrc.size()));
     DWF_CUDA_CHECK(c, cudaMalloc(&s->order, order.size() * sizeof(uint32_t)));

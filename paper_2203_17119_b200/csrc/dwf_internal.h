@@ -58,6 +58,8 @@ struct dwf_ctx {
     int dhop_kernel = 0;   // 0 = auto (TMA kernel for 4^4 tiles, else cp.async tile kernel, else generic), 1 = generic, 2 = cp.async tile kernel
     int dhop_nst = 3;      // ring depth of the pipelined fp32 kernel
     int dhop_grid = 0;     // CTAs of the persistent TMA kernel (0 = SMs x resident CTAs)
+    int dhop_order = 0;    // tile traversal of the TMA kernel: blob extents in tiles as digits (0 = default), dwf_dhop_tma.cu
+    int dhop_order_axes = 0;   // blob path, fastest-first axis digits
     void* tma = nullptr;   // dwf::TmaState (dwf_dhop_tma.cu), built at dwf_set_gauge for 4^4 tiles
     // tables of the pipelined Dhop kernel (dwf_dhop_pipe.cu), built at dwf_set_gauge
     uint16_t* pipe_nbslot = nullptr;
