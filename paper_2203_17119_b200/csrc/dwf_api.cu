@@ -56,6 +56,16 @@ dwf_status mpc_apply(dwf_ctx* c, void* out, const void* in, int dagger, int prec
     void *t1, *t2;
     DWF_TRY(ws_get(c, prec, 0, &t1));
     DWF_TRY(ws_get(c, prec, 1, &t2));
+    if (dhop_fused_available(c)) {
+        // the 5-D operators ride on the Dhop kernels as epilogues (3 / 2 kernels instead of 5 / 4)
+        if (!dagger) {
+            DWF_TRY(launch_op5(c, t1, in, OP_A, nullptr, -1, 0.0, prec, -1));
+            DWF_TRY(launch_dhop_fused(c, t2, t1, DWF_EVEN, 0, prec, EPI_MID, nullptr, 0.0, nullptr, 0, 0, -1));
+            return launch_dhop_fused(c, out, t2, DWF_ODD, 0, prec, EPI_FINAL, in, -0.25, nullptr, 0, 0, norm_slot);
+        }
+        DWF_TRY(launch_dhop_fused(c, t1, in, DWF_EVEN, 1, prec, EPI_MID, nullptr, 0.0, nullptr, 0, 0, -1));
+        return launch_dhop_fused(c, out, t1, DWF_ODD, 1, prec, EPI_FINAL, in, -0.25, nullptr, 0, 0, norm_slot);
+    }
     if (!dagger) {
         DWF_TRY(launch_op5(c, t1, in, OP_A, nullptr, -1, 0.0, prec, -1));
         DWF_TRY(launch_dhop(c, t2, t1, DWF_EVEN, 0, prec));
@@ -108,9 +118,34 @@ dwf_status cg_iterate(dwf_ctx* c, int prec, void* x, void* r, double target, int
     DWF_TRY(ws_get(c, prec, 4, &q));
     DWF_TRY(ws_get(c, prec, 5, &z));
     const size_t n = half_reals(c);
-    DWF_CUDA_CHECK(c, cudaMemcpyAsync(p, r, half_bytes(c->g, prec), cudaMemcpyDeviceToDevice, c->stream));
     int slot_c = SLOT_C, slot_cn = SLOT_CN;
     double cc = *cval;
+    if (dhop_fused_available(c)) {
+        // 5 kernels per iteration (+ 2 single-block reductions): the four Dhops carry A Mee^-1, Mee p - 1/4 (..) with
+        // |q|^2, Mee^-dag A^dag, and r -= alpha (Mee^dag q - 1/4 A^dag (..)) with |r|^2; one column kernel does
+        // x += alpha p, p = r + beta p and the next A p.  Same operation order as the unfused loop (reading C8).
+        void *t1, *t2;
+        DWF_TRY(ws_get(c, prec, 0, &t1));
+        DWF_TRY(ws_get(c, prec, 1, &t2));
+        DWF_TRY(launch_cg_xp(c, x, p, r, t1, prec, slot_c, SLOT_D, slot_cn, 1));          // p = r, t1 = A p
+        while (cc > target && *iters_io < max_iter) {
+            DWF_TRY(launch_dhop_fused(c, t2, t1, DWF_EVEN, 0, prec, EPI_MID, nullptr, 0.0, nullptr, 0, 0, -1));
+            DWF_TRY(launch_dhop_fused(c, q, t2, DWF_ODD, 0, prec, EPI_FINAL, p, -0.25, nullptr, 0, 0, SLOT_D));
+            DWF_TRY(launch_dhop_fused(c, t1, q, DWF_EVEN, 1, prec, EPI_MID, nullptr, 0.0, nullptr, 0, 0, -1));
+            DWF_TRY(launch_dhop_fused(c, t2, t1, DWF_ODD, 1, prec, EPI_CG, q, -0.25, r, slot_c, SLOT_D, slot_cn));
+            double cn;
+            DWF_TRY(read_slot(c, slot_cn, &cn));
+            ++*iters_io;
+            if (!(cn == cn)) { c->err = "CG: NaN residual"; *cval = cn; return DWF_ECUDA; }
+            DWF_TRY(launch_cg_xp(c, x, p, r, t1, prec, slot_c, SLOT_D, slot_cn, 0));      // x += a p; p = r + b p; t1 = A p
+            cc = cn;
+            if (cn <= target) break;
+            int t = slot_c; slot_c = slot_cn; slot_cn = t;
+        }
+        *cval = cc;
+        return DWF_OK;
+    }
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(p, r, half_bytes(c->g, prec), cudaMemcpyDeviceToDevice, c->stream));
     while (cc > target && *iters_io < max_iter) {
         DWF_TRY(mpc_apply(c, q, p, 0, prec, SLOT_D));                 // q = Mpc p, d = |q|^2
         DWF_TRY(mpc_apply(c, z, q, 1, prec, -1));                     // z = Mpc^dag q
@@ -367,11 +402,15 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
         (k == "dhop_order" ? c->dhop_order : c->dhop_order_axes) = (int)val;
         if (c->gauge_set) DWF_TRY(tma_state_build(c));
     }
+    else if (k == "fuse") c->fuse = (val != 0.0);
+    else if (k == "dhop_l2hint") { if (val < 0 || val > 2) return DWF_EINVAL; c->dhop_l2hint = (int)val; }
+    else if (k == "dhop_dynamic") { if (val < 0 || val > 2) return DWF_EINVAL; c->dhop_dynamic = (int)val; }
     else if (k == "dhop_nst") { if (val != 2 && val != 3) return DWF_EINVAL; c->dhop_nst = (int)val; }
     else if (k == "time_dhop") {       // (re)start per-launch event timing of the Dhop kernel
         DWF_TRY(dhop_timing_flush(c));
         c->time_dhop = (val != 0.0);
         c->dhop_ms = 0.0;
+        c->dhop_bytes = 0.0;
         c->dhop_timed = 0;
     }
     else { c->err = "unknown option '" + k + "'"; return DWF_EINVAL; }
@@ -381,10 +420,10 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
 dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
     if (!c || !key || !val) return DWF_EINVAL;
     const std::string k(key);
-    if (k == "dhop_ms" || k == "dhop_timed") {   // synchronises: folds the pending event pairs
+    if (k == "dhop_ms" || k == "dhop_timed" || k == "dhop_bytes") {   // synchronises: folds the pending event pairs
         dwf_ctx* m = const_cast<dwf_ctx*>(c);
         DWF_TRY(dhop_timing_flush(m));
-        *val = (k == "dhop_ms") ? m->dhop_ms : (double)m->dhop_timed;
+        *val = (k == "dhop_ms") ? m->dhop_ms : (k == "dhop_bytes" ? m->dhop_bytes : (double)m->dhop_timed);
         return DWF_OK;
     }
     if (k == "antiperiodic_t") *val = c->g.antiperiodic_t;
@@ -401,6 +440,10 @@ dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
     else if (k == "dhop_kernel") *val = c->dhop_kernel;
     else if (k == "dhop_nst") *val = c->dhop_nst;
     else if (k == "dhop_grid") *val = c->dhop_grid;
+    else if (k == "dhop_dynamic") *val = c->dhop_dynamic;
+    else if (k == "dhop_l2hint") *val = c->dhop_l2hint;
+    else if (k == "fuse") *val = c->fuse;
+    else if (k == "fused_active") *val = dhop_fused_available(c) ? 1.0 : 0.0;
     else if (k == "dhop_order") *val = c->dhop_order;
     else if (k == "dhop_order_axes") *val = c->dhop_order_axes;
     else return DWF_EINVAL;

@@ -146,9 +146,10 @@ dwf_status dhop_timing_flush(dwf_ctx* c) {
 
 static dwf_status launch_dhop_untimed(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec);
 
-// half-field Dhop: out has parity out_parity, in has the other parity
-dwf_status launch_dhop(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec) {
-    if (!c->time_dhop) return launch_dhop_untimed(c, out, in, out_parity, dagger, prec);
+// per-launch CUDA-event timing of the Dhop kernels ("time_dhop"): events on the launching stream around the launch;
+// alg_bytes = algorithmic bytes of this launch, summed for bench.py's roofline
+dwf_status dhop_time_begin(dwf_ctx* c) {
+    if (!c->time_dhop) return DWF_OK;
     const int POOL = 2048;
     if (c->ev.empty()) {
         c->ev.resize(POOL);
@@ -159,10 +160,24 @@ dwf_status launch_dhop(dwf_ctx* c, void* out, const void* in, int out_parity, in
         if (st != DWF_OK) return st;
     }
     DWF_CUDA_CHECK(c, cudaEventRecord(c->ev[c->ev_used], c->stream));
-    dwf_status st = launch_dhop_untimed(c, out, in, out_parity, dagger, prec);
+    return DWF_OK;
+}
+dwf_status dhop_time_end(dwf_ctx* c, double alg_bytes) {
+    if (!c->time_dhop) return DWF_OK;
     DWF_CUDA_CHECK(c, cudaEventRecord(c->ev[c->ev_used + 1], c->stream));
     c->ev_used += 2;
-    return st;
+    c->dhop_bytes += alg_bytes;
+    return DWF_OK;
+}
+
+// half-field Dhop: out has parity out_parity, in has the other parity
+dwf_status launch_dhop(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec) {
+    dwf_status st = dhop_time_begin(c);
+    if (st != DWF_OK) return st;
+    st = launch_dhop_untimed(c, out, in, out_parity, dagger, prec);
+    if (st != DWF_OK) return st;
+    const double B = (prec == DWF_F64) ? 8.0 : 4.0;
+    return dhop_time_end(c, 2.0 * half_bytes(c->g, prec) + (double)c->g.Vh * 8 * (c->compress12 ? 12 : 18) * B);
 }
 
 static dwf_status launch_dhop_untimed(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec) {

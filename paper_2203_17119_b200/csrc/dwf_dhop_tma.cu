@@ -23,6 +23,7 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdint>
 #include <cstring>
 #include <vector>
@@ -157,6 +158,7 @@ struct TmaState {
     uint16_t* off = nullptr;      // device [2][8][128]
     uint8_t* xsrc = nullptr;      // device [2][2][32]
     uint32_t* order = nullptr;    // device [ntiles]
+    int* counters = nullptr;      // device [3]: next position in `order`, CTAs done, round arrivals (self-resetting, see the kernel)
     int K_built = 0;
     int num_sms = 0;
     struct Maps { const void* ptr; int prec; CUtensorMap m[3]; };
@@ -169,6 +171,7 @@ void tma_state_free(dwf_ctx* c) {
     if (s->off) cudaFree(s->off);
     if (s->xsrc) cudaFree(s->xsrc);
     if (s->order) cudaFree(s->order);
+    if (s->counters) cudaFree(s->counters);
     delete s;
     c->tma = nullptr;
 }
@@ -197,6 +200,8 @@ dwf_status tma_state_build(dwf_ctx* c) {
     DWF_CUDA_CHECK(c, cudaMemcpy(s->off, off.data(), off.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
     DWF_CUDA_CHECK(c, cudaMemcpy(s->xsrc, t64.xsrc.data(), t64.xsrc.size(), cudaMemcpyHostToDevice));
     DWF_CUDA_CHECK(c, cudaMemcpy(s->order, order.data(), order.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    DWF_CUDA_CHECK(c, cudaMalloc(&s->counters, 4 * sizeof(int)));
+    DWF_CUDA_CHECK(c, cudaMemset(s->counters, 0, 4 * sizeof(int)));
     return DWF_OK;
 }
 
@@ -282,6 +287,32 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
                  ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
 }
+__device__ __forceinline__ uint64_t l2_policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_normal() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t l2_policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void cp_async16_hint(uint32_t dst, const void* src, uint64_t pol) {
+    asm volatile("cp.async.cg.shared.global.L2::cache_hint [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d_hint(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;"
+                 ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void tma_load_4d_hint(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, uint32_t bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4, %5}], [%6], %7;"
+                 ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar), "l"(pol) : "memory");
+}
 __device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
@@ -352,6 +383,63 @@ __device__ __forceinline__ void recon_s(const R (&g)[12], R s, R (&acc)[24]) {
     }
 }
 
+
+// ------------------------------------------------------------------------------------------ fused 5-D epilogues
+// After the s loop of a tile every consumer thread re-reads the Ls-columns it has just stored itself (they sit in L2),
+// applies the site-local 5-D operator that follows the Dhop in the Schur operator and stores the final values.
+// All 5-D operators are a + b S or (a + b S)^-1 on one chirality, S the s-shift with the -mf wall (readings C4, C5):
+//     (S x)_j = x_{j-1},  (S x)_0 = -mf x_{Ls-1}       in SWEEP order j,
+// where j = s for P+ components and j = Ls-1-s for P- components (daggered operators: the other way round), so one
+// code path serves both chiralities.  A = b5 + c5 S, Mee = bee - cee S.
+// (a + b S)^-1 x:  z_0 = x_0/a, z_j = x_j/a + rho z_{j-1} (rho = -b/a);  G = z_{Ls-1} / (1 + mf rho^Ls);
+//                  y_j = z_j - mf rho^{j+1} G   (so y_{Ls-1} = G).
+struct EpiArgs {
+    int mode;              // EPI_*
+    const void* xin;       // EPI_FINAL / EPI_CG: the field Mee acts on (output parity)
+    void* r;               // EPI_CG: residual, updated in place
+    const double* sc;      // device scalars
+    int slot_c, slot_d;    // EPI_CG: alpha = sc[slot_c] / sc[slot_d]
+    double* partials;      // per-CTA partial sums of |out|^2 (EPI_FINAL) or |r|^2 (EPI_CG); null: none
+    double b5, c5, bee, mcee, mf, scale;     // A = b5 + c5 S ; Mee = bee + mcee S
+    double inva, rho, g0;                    // (bee + mcee S)^-1: 1/bee, cee/bee, 1/(1 + mf rho^Ls)
+    double cj[16];                           // mf rho^{j+1}
+};
+
+__device__ __forceinline__ float4 vmul(float a, const float4& x) { return make_float4(a * x.x, a * x.y, a * x.z, a * x.w); }
+__device__ __forceinline__ double2 vmul(double a, const double2& x) { return make_double2(a * x.x, a * x.y); }
+__device__ __forceinline__ float4 vfma(float a, const float4& x, const float4& y) {
+    return make_float4(fmaf(a, x.x, y.x), fmaf(a, x.y, y.y), fmaf(a, x.z, y.z), fmaf(a, x.w, y.w));
+}
+__device__ __forceinline__ double2 vfma(double a, const double2& x, const double2& y) {
+    return make_double2(fma(a, x.x, y.x), fma(a, x.y, y.y));
+}
+__device__ __forceinline__ double vnorm2(const float4& a) {
+    return (double)a.x * a.x + (double)a.y * a.y + (double)a.z * a.z + (double)a.w * a.w;
+}
+__device__ __forceinline__ double vnorm2(const double2& a) { return a.x * a.x + a.y * a.y; }
+__device__ __forceinline__ float4 ldcs_v(const float4* p) { return __ldcs(p); }
+__device__ __forceinline__ double2 ldcs_v(const double2* p) { return __ldcs(p); }
+
+// y = (a + b S)^-1 x in place, x in sweep order
+template <typename R, typename V, int LS>
+__device__ __forceinline__ void col_inv(V (&x)[LS], R inva, R rho, R g0, const R (&cj)[LS]) {
+    x[0] = vmul(inva, x[0]);
+#pragma unroll
+    for (int j = 1; j < LS; ++j) x[j] = vfma(rho, x[j - 1], vmul(inva, x[j]));
+    const V G = vmul(g0, x[LS - 1]);
+#pragma unroll
+    for (int j = 0; j < LS - 1; ++j) x[j] = vfma(-cj[j], G, x[j]);
+    x[LS - 1] = G;
+}
+// y = (a + b S) x in place (descending so that x_{j-1} is still the input)
+template <typename R, typename V, int LS>
+__device__ __forceinline__ void col_bidiag(V (&x)[LS], R a, R b, R mf) {
+    const V wall = vmul(-mf * b, x[LS - 1]);
+#pragma unroll
+    for (int j = LS - 1; j >= 1; --j) x[j] = vfma(b, x[j - 1], vmul(a, x[j]));
+    x[0] = vfma(a, x[0], wall);
+}
+
 struct TmaArgs {
     Geom g;
     const void* in;
@@ -360,10 +448,102 @@ struct TmaArgs {
     const uint16_t* off;      // [8][128]   (this output parity, this precision)
     const uint8_t* xsrc;      // [2][32]    (this output parity)
     const uint32_t* order;    // [ntiles]
+    int* counters;            // [3] queue / done / round-arrival counters
+    EpiArgs epi;
+    int l2hint;
+    int mode;                 // 0: static round-robin, 1: global in-order queue, 2: static rounds, producers in lockstep
     int dagger;
 };
 
-template <typename R, int TPS, int NG, int NST, int MINB>
+
+// the epilogue of one tile for one consumer thread: its 6 vectors per slice (fp32: all of its site's; fp64: the chirality
+// half it holds), column by column
+template <typename R, int TPS, int LS>
+__device__ __forceinline__ void epilogue(const TmaArgs& a, typename VT<R>::V* __restrict__ outp, int tile, int site, int sub,
+                                         double& nrm) {
+    using V = typename VT<R>::V;
+    constexpr int K = VT<R>::K;
+    constexpr size_t STR = (size_t)K * TSV;          // s stride of a column, in vectors
+    const EpiArgs& e = a.epi;
+    const bool dag = a.dagger != 0;
+    const int k0 = (TPS == 1) ? 0 : sub * 6;
+    const R b5 = (R)e.b5, c5 = (R)e.c5, mf = (R)e.mf;
+    if (e.mode == EPI_MID) {
+        R cj[LS];
+#pragma unroll
+        for (int j = 0; j < LS; ++j) cj[j] = (R)e.cj[j];
+        const R inva = (R)e.inva, rho = (R)e.rho, g0 = (R)e.g0;
+#pragma unroll
+        for (int kb = 0; kb < 6; kb += 2) {
+            V col[2][LS];
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const bool minus = (TPS == 1) ? (kb + q >= 3) : (sub != 0);
+                const bool rev = minus != dag;
+                V* cp = outp + (size_t)(k0 + kb + q) * TSV;
+#pragma unroll
+                for (int j = 0; j < LS; ++j) col[q][j] = cp[(size_t)(rev ? LS - 1 - j : j) * STR];
+            }
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                if (!dag) { col_inv<R, V, LS>(col[q], inva, rho, g0, cj); col_bidiag<R, V, LS>(col[q], b5, c5, mf); }
+                else      { col_bidiag<R, V, LS>(col[q], b5, c5, mf); col_inv<R, V, LS>(col[q], inva, rho, g0, cj); }
+            }
+#pragma unroll
+            for (int q = 0; q < 2; ++q) {
+                const bool minus = (TPS == 1) ? (kb + q >= 3) : (sub != 0);
+                const bool rev = minus != dag;
+                V* cp = outp + (size_t)(k0 + kb + q) * TSV;
+#pragma unroll
+                for (int j = 0; j < LS; ++j) stcs_v(cp + (size_t)(rev ? LS - 1 - j : j) * STR, col[q][j]);
+            }
+        }
+        return;
+    }
+    // EPI_FINAL / EPI_CG
+    const R bee = (R)e.bee, mcee = (R)e.mcee, scale = (R)e.scale;
+    const size_t toff = (size_t)tile * LS * STR + site;
+    const V* __restrict__ xin = reinterpret_cast<const V*>(e.xin) + toff;
+    V* __restrict__ rres = reinterpret_cast<V*>(e.r) + toff;
+    R alpha = (R)0;
+    if (e.mode == EPI_CG) alpha = (R)(e.sc[e.slot_c] / e.sc[e.slot_d]);
+#pragma unroll
+    for (int kk = 0; kk < 6; ++kk) {
+        const bool minus = (TPS == 1) ? (kk >= 3) : (sub != 0);
+        const bool rev = minus != dag;
+        V* cp = outp + (size_t)(k0 + kk) * TSV;
+        const V* xp = xin + (size_t)(k0 + kk) * TSV;
+        V d[LS], x[LS];
+#pragma unroll
+        for (int j = 0; j < LS; ++j) {
+            const size_t o = (size_t)(rev ? LS - 1 - j : j) * STR;
+            d[j] = cp[o];
+            x[j] = ldcs_v(xp + o);
+        }
+        if (dag) col_bidiag<R, V, LS>(d, b5, c5, mf);      // A^dag on the hopping term
+        col_bidiag<R, V, LS>(x, bee, mcee, mf);             // Mee (Mee^dag) on the diagonal term
+        if (e.mode == EPI_FINAL) {
+#pragma unroll
+            for (int j = 0; j < LS; ++j) {
+                const V o = vfma(scale, d[j], x[j]);
+                nrm += vnorm2(o);
+                stcs_v(cp + (size_t)(rev ? LS - 1 - j : j) * STR, o);
+            }
+        } else {
+            V* rp = rres + (size_t)(k0 + kk) * TSV;
+#pragma unroll
+            for (int j = 0; j < LS; ++j) {
+                const size_t o = (size_t)(rev ? LS - 1 - j : j) * STR;
+                const V z = vfma(scale, d[j], x[j]);
+                const V rn = vfma(-alpha, z, rp[o]);
+                nrm += vnorm2(rn);
+                rp[o] = rn;
+            }
+        }
+    }
+}
+
+template <typename R, int TPS, int NG, int NST, int MINB, int LS>
 __global__ void __launch_bounds__(128 + 128 * TPS, MINB)
 dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, const __grid_constant__ CUtensorMap map_z,
                 const __grid_constant__ CUtensorMap map_y) {
@@ -379,6 +559,7 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
 
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[2 * NST];   // full[NST], empty[NST]
+    __shared__ int next_of[4];     // slot j & 3, written before slice 0 of this CTA's j-th tile: the tile it takes after it (-1: none)
 
     const Geom& g = a.g;
     const int Ls = g.Ls;
@@ -406,9 +587,34 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
         const V* __restrict__ in = reinterpret_cast<const V*>(a.in);
         const unsigned xs_p = a.xsrc[lane], xs_m = a.xsrc[32 + lane];
         const uint32_t tile_vecs = (uint32_t)Ls * K * TSV;
-        uint32_t n = 0;
-        for (int it = blockIdx.x; it < ntiles; it += gridDim.x) {
+        uint32_t n = 0, j = 0;
+        int it = blockIdx.x;
+        // L2 policy of every read of the input field: its sectors are wanted again (as a neighbour's face or as the
+        // owner's slab), unlike the links and the output, which stream through once
+        const uint64_t pol = (a.l2hint == 1) ? l2_policy_evict_last() : (a.l2hint == 2 ? l2_policy_evict_first() : l2_policy_evict_normal());
+        while (it < ntiles) {
+            // next position in `order`: static round-robin, or the global in-order queue (tiles start in `order`
+            // sequence whatever the CTAs' speeds, which keeps neighbouring tiles in phase: their faces hit L2)
+            int it_next = it + gridDim.x;
+            if (a.mode == 2 && j > 0) {
+                // lockstep rounds: every producer arrives, then waits until all have (CTAs are co-resident: grid =
+                // SMs x resident CTAs; the bounded spin makes a missing CTA cost time, never a hang).  Producers run
+                // up to NST slices ahead of their consumers, which hides the wait.
+                if (lane == 0) {
+                    atomicAdd(a.counters + 2, 1);
+                    const int target = (int)gridDim.x * (int)j;
+                    const long long t0 = clock64();
+                    while (*(volatile int*)(a.counters + 2) < target && clock64() - t0 < 4000000LL) __nanosleep(64);
+                }
+                __syncwarp();
+            }
+            if (a.mode == 1) {
+                int v = 0;
+                if (lane == 0) v = atomicAdd(a.counters, 1) + (int)gridDim.x;
+                it_next = __shfl_sync(0xffffffffu, v, 0);
+            }
             const int tile = a.order[it];
+            const int tile_next = (it_next < ntiles) ? (int)a.order[it_next] : -1;
             int tc[4];
             tile_coords(g, tile, tc);
             int nt[8];
@@ -420,10 +626,12 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                 nc[mu] = (tc[mu] == 0) ? g.NT[mu] - 1 : tc[mu] - 1;
                 nt[2 * mu + 1] = tile_index(g, nc);
             }
-            if (lane == 0 && it + (int)gridDim.x < ntiles) {     // next tile's links -> L2
-                const int nx = a.order[it + gridDim.x];
-                l2_prefetch_bulk(reinterpret_cast<const V*>(a.W) + (size_t)nx * 8 * KG * TSV, 8 * KG * TSV * 16);
+            if (lane == 0) {
+                next_of[j & 3] = tile_next;       // published by the release-arrive on slice 0's `full` barrier
+                if (tile_next >= 0)               // next tile's links -> L2
+                    l2_prefetch_bulk(reinterpret_cast<const V*>(a.W) + (size_t)tile_next * 8 * KG * TSV, 8 * KG * TSV * 16);
             }
+            ++j;
             const V* src_p = in + (size_t)nt[0] * tile_vecs + xs_p;
             const V* src_m = in + (size_t)nt[1] * tile_vecs + xs_m;
             for (int s = 0; s < Ls; ++s, ++n) {
@@ -435,23 +643,34 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                     mbar_arrive_expect_tx(full, 10 * REGION_BYTES);
                     const int row_own = (tile * Ls + s) * K;
 #pragma unroll
-                    for (int tt = 0; tt < 4; ++tt) tma_load_3d(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full);
-                    tma_load_3d(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full);
-                    tma_load_3d(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full);
-                    tma_load_4d(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full);
-                    tma_load_4d(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full);
-                    tma_load_4d(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full);
-                    tma_load_4d(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full);
+                    for (int tt = 0; tt < 4; ++tt) tma_load_3d_hint(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full, pol);
+                    tma_load_3d_hint(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full, pol);
+                    tma_load_3d_hint(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full, pol);
+                    tma_load_4d_hint(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full, pol);
+                    tma_load_4d_hint(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full, pol);
+                    tma_load_4d_hint(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full, pol);
+                    tma_load_4d_hint(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full, pol);
                 }
                 const V* sp = src_p + (size_t)s * (K * TSV);
                 const V* sm = src_m + (size_t)s * (K * TSV);
                 const uint32_t dp = base + 10 * REGION_BYTES + lane * 16, dm = base + 11 * REGION_BYTES + lane * 16;
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-                    cp_async16_tma(dp + k * 512, sp + k * TSV);
-                    cp_async16_tma(dm + k * 512, sm + k * TSV);
+                    cp_async16_hint(dp + k * 512, sp + k * TSV, pol);
+                    cp_async16_hint(dm + k * 512, sm + k * TSV, pol);
                 }
                 cp_async_mbar_arrive_noinc(full);
+            }
+            it = it_next;
+        }
+        if (a.mode != 0 && lane == 0) {          // the last CTA out re-arms the counters for the next launch
+            const uint32_t nrounds = ((uint32_t)ntiles + gridDim.x - 1) / gridDim.x;
+            if (a.mode == 2 && j < nrounds) atomicAdd(a.counters + 2, 1);     // no tile in the last round: arrive anyway
+            __threadfence();
+            if (atomicAdd(a.counters + 1, 1) == (int)gridDim.x - 1) {
+                atomicExch(a.counters, 0);
+                atomicExch(a.counters + 1, 0);
+                atomicExch(a.counters + 2, 0);
             }
         }
         return;
@@ -473,9 +692,11 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
     }
     const int tt = site >> 5;
     const R dsgn = a.dagger ? (R)-1 : (R)1;
-    uint32_t n = 0;
-    for (int it = blockIdx.x; it < ntiles; it += gridDim.x) {
-        const int tile = a.order[it];
+    uint32_t n = 0, j = 0;
+    double nrm = 0.0;
+    int tile = a.order[blockIdx.x];
+    while (tile >= 0) {
+        int tile_next = -1;
         const int tct = tile / (g.NT[0] * g.NT[1] * g.NT[2]);
         const int tglob = tct * 4 + tt;
         // ---- links to registers (once per tile): rows 0,1 (+ row 2 rebuilt), antiperiodic sign folded in
@@ -502,6 +723,7 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
             const uint32_t st = n % NST, ph = (n / NST) & 1;
             const uint32_t base = stage0 + st * STAGE_BYTES;
             mbar_wait(bar0 + 8 * st, ph);
+            if (s == 0) tile_next = *(volatile int*)&next_of[j & 3];
             R acc[24];
 #pragma unroll
             for (int j = 0; j < LPT; ++j) {
@@ -521,9 +743,15 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
             __syncwarp();
             if (lane == 0) mbar_arrive(bar0 + 8 * (NST + st));      // stage released
             V* o = outp + (size_t)s * (K * TSV);
+            const bool keep = (LS > 0) && a.epi.mode != EPI_NONE;      // the epilogue re-reads the tile from L2
             if (TPS == 1) {
+                if (keep) {
 #pragma unroll
-                for (int k = 0; k < K; ++k) stcs_v(o + k * TSV, packv(acc + k * VW));
+                    for (int k = 0; k < K; ++k) o[k * TSV] = packv(acc + k * VW);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < K; ++k) stcs_v(o + k * TSV, packv(acc + k * VW));
+                }
             } else {
                 // lane pair (l, l^16): each keeps one chirality half of the 24 sums, sends the other
                 R mine[12];
@@ -534,19 +762,43 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                     mine[i] = keep + shfl16(send);
                 }
                 V* o2 = o + (sub ? (K / 2) * TSV : 0);
+                if (keep) {
 #pragma unroll
-                for (int k = 0; k < K / 2; ++k) stcs_v(o2 + k * TSV, packv(mine + k * VW));
+                    for (int k = 0; k < K / 2; ++k) o2[k * TSV] = packv(mine + k * VW);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < K / 2; ++k) stcs_v(o2 + k * TSV, packv(mine + k * VW));
+                }
             }
+        }
+        if constexpr (LS > 0) {
+            if (a.epi.mode != EPI_NONE) epilogue<R, TPS, LS>(a, outp, tile, site, sub, nrm);
+        }
+        tile = tile_next;
+        ++j;
+    }
+    if (LS > 0 && a.epi.mode >= EPI_FINAL && a.epi.partials != nullptr) {
+        // fixed-tree sum over the consumer threads (static tile assignment: bit-reproducible run to run)
+        __shared__ double wsum[NCW];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
+        if (lane == 0) wsum[cw] = nrm;
+        asm volatile("bar.sync 1, %0;" ::"n"(128 * TPS) : "memory");
+        if (ctid == 0) {
+            double t = 0.0;
+#pragma unroll
+            for (int i = 0; i < NCW; ++i) t += wsum[i];
+            a.epi.partials[blockIdx.x] = t;
         }
     }
 }
 
 // ------------------------------------------------------------------------------------------ launch
-template <typename R, int TPS, int NG, int NST, int MINB>
-static dwf_status launch_tma_t(dwf_ctx* c, const TmaArgs& a, const CUtensorMap* maps) {
+template <typename R, int TPS, int NG, int NST, int MINB, int LS>
+static dwf_status launch_tma_t(dwf_ctx* c, const TmaArgs& a, const CUtensorMap* maps, int* grid_out) {
     constexpr int K = VT<R>::K;
     const size_t smem = (size_t)NST * NREG * K * 512;
-    auto kern = dhop_tma_kernel<R, TPS, NG, NST, MINB>;
+    auto kern = dhop_tma_kernel<R, TPS, NG, NST, MINB, LS>;
     static bool attr_done = false;
     if (!attr_done) {
         DWF_CUDA_CHECK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -556,30 +808,93 @@ static dwf_status launch_tma_t(dwf_ctx* c, const TmaArgs& a, const CUtensorMap* 
     int grid = s->num_sms * MINB;
     if (c->dhop_grid > 0) grid = c->dhop_grid;
     if (grid > c->g.ntiles) grid = c->g.ntiles;
+    if (grid_out) *grid_out = grid;
     kern<<<grid, 128 + 128 * TPS, smem, c->stream>>>(a, maps[0], maps[1], maps[2]);
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
     return DWF_OK;
 }
 
-dwf_status launch_dhop_tma(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, bool* handled) {
-    *handled = false;
+static dwf_status fill_args(dwf_ctx* c, TmaArgs& a, void* out, const void* in, int out_parity, int dagger, int prec,
+                            const CUtensorMap** maps) {
     TmaState* s = (TmaState*)c->tma;
-    if (!s) return DWF_OK;
-    const CUtensorMap* maps = nullptr;
-    dwf_status st = get_maps(c, in, prec, &maps);
+    dwf_status st = get_maps(c, in, prec, maps);
     if (st != DWF_OK) return st;
-    TmaArgs a;
+    memset(&a, 0, sizeof(a));
     a.g = c->g; a.in = in; a.out = out;
     a.W = (prec == DWF_F64) ? c->W64[out_parity] : c->W32[out_parity];
     a.off = s->off + (size_t)(prec == DWF_F64 ? 0 : 2 * 8 * TSV) + (size_t)out_parity * 8 * TSV;
     a.xsrc = s->xsrc + (size_t)out_parity * 2 * 32;
     a.order = s->order;
+    a.counters = s->counters;
+    a.mode = c->dhop_dynamic;
+    a.l2hint = c->dhop_l2hint;
     a.dagger = dagger;
+    a.epi.mode = EPI_NONE;
+    return DWF_OK;
+}
+
+dwf_status launch_dhop_tma(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, bool* handled) {
+    *handled = false;
+    if (!c->tma) return DWF_OK;
+    const CUtensorMap* maps = nullptr;
+    TmaArgs a;
+    dwf_status st = fill_args(c, a, out, in, out_parity, dagger, prec, &maps);
+    if (st != DWF_OK) return st;
     *handled = true;
     if (prec == DWF_F64)
-        return c->compress12 ? launch_tma_t<double, 2, 12, 3, 1>(c, a, maps) : launch_tma_t<double, 2, 18, 3, 1>(c, a, maps);
-    return c->compress12 ? launch_tma_t<float, 1, 12, 3, 2>(c, a, maps) : launch_tma_t<float, 1, 18, 3, 2>(c, a, maps);
+        return c->compress12 ? launch_tma_t<double, 2, 12, 3, 1, 0>(c, a, maps, nullptr)
+                             : launch_tma_t<double, 2, 18, 3, 1, 0>(c, a, maps, nullptr);
+    return c->compress12 ? launch_tma_t<float, 1, 12, 3, 2, 0>(c, a, maps, nullptr)
+                         : launch_tma_t<float, 1, 18, 3, 2, 0>(c, a, maps, nullptr);
+}
+
+// the fused kernels exist for 4^4 tiles, 2-row links and Ls = 8, 12, 16 (the Ls column lives in registers)
+bool dhop_fused_available(const dwf_ctx* c) {
+    return c->tma != nullptr && c->fuse && c->compress12 && (c->g.Ls == 8 || c->g.Ls == 12 || c->g.Ls == 16);
+}
+
+dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, int epi,
+                             const void* xin, double scale, void* r, int slot_c, int slot_d, int norm_slot) {
+    if (!dhop_fused_available(c)) { c->err = "fused Dhop kernel not available for this geometry"; return DWF_ESTATE; }
+    const CUtensorMap* maps = nullptr;
+    TmaArgs a;
+    dwf_status st = fill_args(c, a, out, in, out_parity, dagger, prec, &maps);
+    if (st != DWF_OK) return st;
+    const int Ls = c->g.Ls;
+    const double bee = 1.0 + c->b5 * (4.0 - c->M5), cee = 1.0 - c->c5 * (4.0 - c->M5);
+    EpiArgs& e = a.epi;
+    e.mode = epi;
+    e.xin = xin; e.r = r; e.sc = c->scalars; e.slot_c = slot_c; e.slot_d = slot_d;
+    e.b5 = c->b5; e.c5 = c->c5; e.bee = bee; e.mcee = -cee; e.mf = c->mf; e.scale = scale;
+    e.inva = 1.0 / bee; e.rho = cee / bee; e.g0 = 1.0 / (1.0 + c->mf * std::pow(e.rho, Ls));
+    for (int j = 0; j < 16; ++j) e.cj[j] = (j < Ls) ? c->mf * std::pow(e.rho, j + 1) : 0.0;
+    a.mode = 0;                                    // static tile assignment: reproducible reductions
+    int grid = 0;
+    st = dhop_time_begin(c);
+    if (st != DWF_OK) return st;
+    if (norm_slot >= 0) {
+        TmaState* s = (TmaState*)c->tma;
+        st = ensure_partials(c, s->num_sms * 2);
+        if (st != DWF_OK) return st;
+        e.partials = c->partials;
+    }
+#define DWF_FUSED(LSV)                                                                                     \
+    st = (prec == DWF_F64) ? launch_tma_t<double, 2, 12, 3, 1, LSV>(c, a, maps, &grid)                     \
+                           : launch_tma_t<float, 1, 12, 3, 2, LSV>(c, a, maps, &grid)
+    if (Ls == 8) DWF_FUSED(8);
+    else if (Ls == 12) DWF_FUSED(12);
+    else DWF_FUSED(16);
+#undef DWF_FUSED
+    if (st != DWF_OK) return st;
+    {   // algorithmic bytes: the input field, the links, the extra epilogue operands, one field written
+        const double S = (double)half_bytes(c->g, prec), B = (prec == DWF_F64) ? 8.0 : 4.0;
+        const double nfields = (epi == EPI_MID) ? 2.0 : (epi == EPI_FINAL ? 3.0 : 4.0);
+        st = dhop_time_end(c, nfields * S + (double)c->g.Vh * 8 * 12 * B);
+        if (st != DWF_OK) return st;
+    }
+    if (norm_slot >= 0) return launch_reduce(c, grid, norm_slot);
+    return DWF_OK;
 }
 
 }  // namespace dwf

@@ -75,6 +75,8 @@ __device__ __forceinline__ void fmav(float4& a, float t, const float4& x) {
 __device__ __forceinline__ void fmav(double2& a, double t, const double2& x) {
     a.x = fma(t, x.x, a.x); a.y = fma(t, x.y, a.y);
 }
+__device__ __forceinline__ void scalev(float4& a, float t) { a.x *= t; a.y *= t; a.z *= t; a.w *= t; }
+__device__ __forceinline__ void scalev(double2& a, double t) { a.x *= t; a.y *= t; }
 __device__ __forceinline__ float4 zerov(float4*) { return make_float4(0.f, 0.f, 0.f, 0.f); }
 __device__ __forceinline__ double2 zerov(double2*) { return make_double2(0.0, 0.0); }
 __device__ __forceinline__ double norm2v(const float4& a) {
@@ -175,6 +177,76 @@ __global__ void __launch_bounds__(128) op5_kernel(int Ls_rt, int TS, unsigned nv
         double tot = block_reduce_sum(nrm);
         if (threadIdx.x == 0) partials[blockIdx.x] = tot;
     }
+}
+
+
+// CG vector step fused with the next A p (fused CG loop, dwf_api.cu):  x += alpha p;  p <- r + beta p;  ap = A p,
+// A = b5 + c5 Q (reading C5).  One thread owns one 16-byte vector column of one 4-D site and walks it in sweep order
+// (s ascending on P+ components, descending on P-), so (Q p)_j is the previous element, the -mf wall at j = 0.
+// init: p <- r, ap = A p, x untouched.  alpha = sc[slot_c]/sc[slot_d], beta = sc[slot_cn]/sc[slot_c].
+template <typename R>
+__global__ void __launch_bounds__(128) cg_xp_kernel(int Ls, int TS, unsigned nvec_site, typename V5<R>::V* __restrict__ x,
+                                                    typename V5<R>::V* __restrict__ p,
+                                                    const typename V5<R>::V* __restrict__ r,
+                                                    typename V5<R>::V* __restrict__ ap, const double* __restrict__ sc,
+                                                    int slot_c, int slot_d, int slot_cn, int init, R b5, R c5, R mf) {
+    using V = typename V5<R>::V;
+    constexpr int K = V5<R>::K;
+    const unsigned gid = blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= nvec_site) return;
+    const unsigned per_tile = (unsigned)K * TS;
+    const unsigned tile = gid / per_tile, j = gid - tile * per_tile;
+    const int k = j / TS;
+    const bool rev = (k >= K / 2);
+    const size_t base = (size_t)tile * Ls * per_tile + j;
+    R alpha = (R)0, beta = (R)0;
+    if (!init) {
+        const double cc = sc[slot_c];
+        alpha = (R)(cc / sc[slot_d]);
+        beta = (R)(sc[slot_cn] / cc);
+    }
+    const size_t olast = base + (size_t)(rev ? 0 : Ls - 1) * per_tile;
+    V prev = r[olast];
+    if (!init) fmav(prev, beta, p[olast]);
+    scalev(prev, -mf);
+#pragma unroll 4
+    for (int jj = 0; jj < Ls; ++jj) {
+        const size_t o = base + (size_t)(rev ? Ls - 1 - jj : jj) * per_tile;
+        V pn = r[o];
+        if (!init) {
+            const V pv = p[o];
+            V xv = x[o];
+            fmav(xv, alpha, pv);
+            x[o] = xv;
+            fmav(pn, beta, pv);
+        }
+        p[o] = pn;
+        V a = zerov((V*)nullptr);
+        fmav(a, b5, pn);
+        fmav(a, c5, prev);
+        ap[o] = a;
+        prev = pn;
+    }
+}
+
+dwf_status launch_cg_xp(dwf_ctx* c, void* x, void* p, const void* r, void* ap, int prec, int slot_c, int slot_d,
+                        int slot_cn, int init) {
+    const Geom& g = c->g;
+    const int block = 128;
+    if (prec == DWF_F64) {
+        const unsigned nvec_site = (unsigned)g.Vh * 12;
+        cg_xp_kernel<double><<<(nvec_site + block - 1) / block, block, 0, c->stream>>>(
+            g.Ls, g.TS, nvec_site, (double2*)x, (double2*)p, (const double2*)r, (double2*)ap, c->scalars, slot_c, slot_d,
+            slot_cn, init, c->b5, c->c5, c->mf);
+    } else {
+        const unsigned nvec_site = (unsigned)g.Vh * 6;
+        cg_xp_kernel<float><<<(nvec_site + block - 1) / block, block, 0, c->stream>>>(
+            g.Ls, g.TS, nvec_site, (float4*)x, (float4*)p, (const float4*)r, (float4*)ap, c->scalars, slot_c, slot_d,
+            slot_cn, init, (float)c->b5, (float)c->c5, (float)c->mf);
+    }
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
 }
 
 // fixed-tree final reduction of the per-block partials into one device scalar

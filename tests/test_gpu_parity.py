@@ -33,11 +33,13 @@ class Case:
     """One lattice: gauge, GPU context(s), fp64 oracle (the fp32 GPU path is compared with the fp64 oracle
     run on the fp32-rounded gauge and source, SURVEY §8(c) 'other silent points' (iii))."""
 
-    def __init__(self, api, dims, Ls, par, eps=0.4, cut=(0, 0, 0, 0), apbc=True, seed=7, compress12=1, tiles=None):
+    def __init__(self, api, dims, Ls, par, eps=0.4, cut=(0, 0, 0, 0), apbc=True, seed=7, compress12=1, tiles=None, fuse=1,
+                 fused=None):
         from oracle.dwf_oracle import Oracle
         self.api, self.dims, self.Ls = api, tuple(dims), Ls
         self.U = inputs.gauge_weak(dims, eps, seed)
-        opts = dict(antiperiodic_t=int(apbc), compress12=compress12)
+        opts = dict(antiperiodic_t=int(apbc), compress12=compress12, fuse=fuse)
+        self.fused = fused
         if tiles:
             opts.update({f"tile_{k}": v for k, v in zip("xyzt", tiles)})
         self.gpu = api.Dwf(dims, Ls, par["M5"], par["mf"], par["b5"], par["c5"], cut=cut, **opts)
@@ -72,13 +74,13 @@ class Case:
 
 CASES = {
     # c1: BASELINE configs[0]
-    "c1": dict(dims=(4, 4, 4, 4), Ls=8, par=SHAM, eps=0.2),
+    "c1": dict(dims=(4, 4, 4, 4), Ls=8, par=SHAM, eps=0.2, fused=True),
     # several tiles + a ragged mix of tile extents (6 -> tiles of 2), Moebius, Ls with a specialised kernel
     "ragged": dict(dims=(8, 4, 6, 12), Ls=12, par=MOEB, eps=0.5),
     # generic-Ls path (Ls = 5 has no unrolled instantiation), periodic t
     "ls5": dict(dims=(4, 8, 4, 4), Ls=5, par=MOEB, eps=0.5, apbc=False),
     # Dirichlet cut in t (c2's geometry scaled down) and a second cut in x
-    "cut": dict(dims=(8, 8, 8, 16), Ls=16, par=MOEB, eps=0.3, cut=(0, 0, 0, 8)),
+    "cut": dict(dims=(8, 8, 8, 16), Ls=16, par=MOEB, eps=0.3, cut=(0, 0, 0, 8), fused=True),
     "cut2": dict(dims=(8, 4, 4, 8), Ls=8, par=MOEB, eps=0.3, cut=(4, 0, 0, 4)),
     # uncompressed 18-real links
     "g18": dict(dims=(4, 4, 8, 8), Ls=8, par=MOEB, eps=0.7, compress12=0),
@@ -86,6 +88,12 @@ CASES = {
     "tiny": dict(dims=(2, 2, 2, 2), Ls=1, par=MOEB, eps=0.7),
     # non-default tiles
     "tiles": dict(dims=(8, 8, 4, 8), Ls=4, par=MOEB, eps=0.7, tiles=(8, 2, 2, 4)),
+    # the fused-epilogue Dhop kernels (4^4 tiles, Ls in {8, 12, 16}) -- c1, cut and cut2 above run them too -- and the
+    # same lattices through the separate 5-D kernels (fuse=0)
+    "fused12": dict(dims=(8, 8, 4, 8), Ls=12, par=MOEB, eps=0.5, fused=True),
+    "fused12_shamir": dict(dims=(4, 8, 8, 4), Ls=12, par=SHAM, eps=0.5, apbc=False, fused=True),
+    "unfused12": dict(dims=(8, 8, 4, 8), Ls=12, par=MOEB, eps=0.5, fuse=0, fused=False),
+    "c1_unfused": dict(dims=(4, 4, 4, 4), Ls=8, par=SHAM, eps=0.2, fuse=0, fused=False),
 }
 
 
@@ -94,6 +102,11 @@ def case(request, api, oracle_built):
     c = Case(api, **CASES[request.param])
     yield c
     c.gpu.close()
+
+
+def test_fused_path_is_the_one_expected(case):
+    if case.fused is not None:
+        assert bool(case.gpu.get_option("fused_active")) == case.fused
 
 
 @pytest.mark.parametrize("prec", ["f64", "f32"])
