@@ -56,15 +56,12 @@ dwf_status mpc_apply(dwf_ctx* c, void* out, const void* in, int dagger, int prec
     void *t1, *t2;
     DWF_TRY(ws_get(c, prec, 0, &t1));
     DWF_TRY(ws_get(c, prec, 1, &t2));
-    if (dhop_fused_available(c)) {
-        // the 5-D operators ride on the Dhop kernels as epilogues (3 / 2 kernels instead of 5 / 4)
-        if (!dagger) {
-            DWF_TRY(launch_op5(c, t1, in, OP_A, nullptr, -1, 0.0, prec, -1));
-            DWF_TRY(launch_dhop_fused(c, t2, t1, DWF_EVEN, 0, prec, EPI_MID, nullptr, 0.0, nullptr, 0, 0, -1));
-            return launch_dhop_fused(c, out, t2, DWF_ODD, 0, prec, EPI_FINAL, in, -0.25, nullptr, 0, 0, norm_slot);
-        }
-        DWF_TRY(launch_dhop_fused(c, t1, in, DWF_EVEN, 1, prec, EPI_MID, nullptr, 0.0, nullptr, 0, 0, -1));
-        return launch_dhop_fused(c, out, t1, DWF_ODD, 1, prec, EPI_FINAL, in, -0.25, nullptr, 0, 0, norm_slot);
+    if (!dagger && dhop_fused_available(c)) {
+        // the last step, Moo in - 1/4 (..) with the optional |.|^2, rides on the second Dhop (4 kernels instead of 5)
+        DWF_TRY(launch_op5(c, t1, in, OP_A, nullptr, -1, 0.0, prec, -1));
+        DWF_TRY(launch_dhop(c, t2, t1, DWF_EVEN, 0, prec));
+        DWF_TRY(launch_op5(c, t1, t2, OP_A_MEEINV, nullptr, -1, 0.0, prec, -1));
+        return launch_dhop_fused(c, out, t1, DWF_ODD, prec, in, -0.25, norm_slot);
     }
     if (!dagger) {
         DWF_TRY(launch_op5(c, t1, in, OP_A, nullptr, -1, 0.0, prec, -1));
@@ -121,18 +118,22 @@ dwf_status cg_iterate(dwf_ctx* c, int prec, void* x, void* r, double target, int
     int slot_c = SLOT_C, slot_cn = SLOT_CN;
     double cc = *cval;
     if (dhop_fused_available(c)) {
-        // 5 kernels per iteration (+ 2 single-block reductions): the four Dhops carry A Mee^-1, Mee p - 1/4 (..) with
-        // |q|^2, Mee^-dag A^dag, and r -= alpha (Mee^dag q - 1/4 A^dag (..)) with |r|^2; one column kernel does
-        // x += alpha p, p = r + beta p and the next A p.  Same operation order as the unfused loop (reading C8).
+        // 8 kernels per iteration moving 23 half fields instead of 11 moving 29: the second Dhop
+        // carries q = Mee p - 1/4 (..) and |q|^2; one column kernel forms z = Mpc^dag's last step in registers and does
+        // r -= alpha z, |r|^2; one does x += alpha p, p = r + beta p and the next A p.  Same operation order as the
+        // unfused loop (reading C8).
         void *t1, *t2;
         DWF_TRY(ws_get(c, prec, 0, &t1));
         DWF_TRY(ws_get(c, prec, 1, &t2));
         DWF_TRY(launch_cg_xp(c, x, p, r, t1, prec, slot_c, SLOT_D, slot_cn, 1));          // p = r, t1 = A p
         while (cc > target && *iters_io < max_iter) {
-            DWF_TRY(launch_dhop_fused(c, t2, t1, DWF_EVEN, 0, prec, EPI_MID, nullptr, 0.0, nullptr, 0, 0, -1));
-            DWF_TRY(launch_dhop_fused(c, q, t2, DWF_ODD, 0, prec, EPI_FINAL, p, -0.25, nullptr, 0, 0, SLOT_D));
-            DWF_TRY(launch_dhop_fused(c, t1, q, DWF_EVEN, 1, prec, EPI_MID, nullptr, 0.0, nullptr, 0, 0, -1));
-            DWF_TRY(launch_dhop_fused(c, t2, t1, DWF_ODD, 1, prec, EPI_CG, q, -0.25, r, slot_c, SLOT_D, slot_cn));
+            DWF_TRY(launch_dhop(c, t2, t1, DWF_EVEN, 0, prec));
+            DWF_TRY(launch_op5(c, t1, t2, OP_A_MEEINV, nullptr, -1, 0.0, prec, -1));
+            DWF_TRY(launch_dhop_fused(c, q, t1, DWF_ODD, prec, p, -0.25, SLOT_D));           // q = Mpc p, d = |q|^2
+            DWF_TRY(launch_dhop(c, t1, q, DWF_EVEN, 1, prec));
+            DWF_TRY(launch_op5(c, t2, t1, OP_MEEINVDAG_ADAG, nullptr, -1, 0.0, prec, -1));
+            DWF_TRY(launch_dhop(c, t1, t2, DWF_ODD, 1, prec));
+            DWF_TRY(launch_cg_r(c, r, q, t1, -0.25, prec, slot_c, SLOT_D, slot_cn));   // r -= a Mpc^dag q
             double cn;
             DWF_TRY(read_slot(c, slot_cn, &cn));
             ++*iters_io;
@@ -403,6 +404,7 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
         if (c->gauge_set) DWF_TRY(tma_state_build(c));
     }
     else if (k == "fuse") c->fuse = (val != 0.0);
+    else if (k == "dhop_skip") c->dhop_skip = (int)val;
     else if (k == "dhop_l2hint") { if (val < 0 || val > 2) return DWF_EINVAL; c->dhop_l2hint = (int)val; }
     else if (k == "dhop_dynamic") { if (val < 0 || val > 2) return DWF_EINVAL; c->dhop_dynamic = (int)val; }
     else if (k == "dhop_nst") { if (val != 2 && val != 3) return DWF_EINVAL; c->dhop_nst = (int)val; }

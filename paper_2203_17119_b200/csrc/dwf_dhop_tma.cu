@@ -313,6 +313,7 @@ __device__ __forceinline__ void tma_load_4d_hint(uint32_t dst, const CUtensorMap
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4, %5}], [%6], %7;"
                  ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar), "l"(pol) : "memory");
 }
+__device__ __forceinline__ void l2_prefetch(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
@@ -327,6 +328,22 @@ __device__ __forceinline__ float4 lds_v(const float4*, uint32_t a) {
 __device__ __forceinline__ double2 lds_v(const double2*, uint32_t a) {
     double2 v;
     asm volatile("ld.shared.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ void st_hint(float4* p, const float4& v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.v4.f32 [%0], {%1,%2,%3,%4}, %5;" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_hint(double2* p, const double2& v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.v2.f64 [%0], {%1,%2}, %3;" ::"l"(p), "d"(v.x), "d"(v.y), "l"(pol) : "memory");
+}
+__device__ __forceinline__ float4 ld_hint(const float4* p, uint64_t pol) {
+    float4 v;
+    asm volatile("ld.global.L2::cache_hint.v4.f32 {%0,%1,%2,%3}, [%4], %5;" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p), "l"(pol) : "memory");
+    return v;
+}
+__device__ __forceinline__ double2 ld_hint(const double2* p, uint64_t pol) {
+    double2 v;
+    asm volatile("ld.global.L2::cache_hint.v2.f64 {%0,%1}, [%2], %3;" : "=d"(v.x), "=d"(v.y) : "l"(p), "l"(pol) : "memory");
     return v;
 }
 __device__ __forceinline__ void stcs_v(float4* p, const float4& v) { __stcs(p, v); }
@@ -384,25 +401,18 @@ __device__ __forceinline__ void recon_s(const R (&g)[12], R s, R (&acc)[24]) {
 }
 
 
-// ------------------------------------------------------------------------------------------ fused 5-D epilogues
-// After the s loop of a tile every consumer thread re-reads the Ls-columns it has just stored itself (they sit in L2),
-// applies the site-local 5-D operator that follows the Dhop in the Schur operator and stores the final values.
-// All 5-D operators are a + b S or (a + b S)^-1 on one chirality, S the s-shift with the -mf wall (readings C4, C5):
-//     (S x)_j = x_{j-1},  (S x)_0 = -mf x_{Ls-1}       in SWEEP order j,
-// where j = s for P+ components and j = Ls-1-s for P- components (daggered operators: the other way round), so one
-// code path serves both chiralities.  A = b5 + c5 S, Mee = bee - cee S.
-// (a + b S)^-1 x:  z_0 = x_0/a, z_j = x_j/a + rho z_{j-1} (rho = -b/a);  G = z_{Ls-1} / (1 + mf rho^Ls);
-//                  y_j = z_j - mf rho^{j+1} G   (so y_{Ls-1} = G).
+// ------------------------------------------------------------------------------------------ fused epilogue
+// The last step of Mpc rides on the Dhop kernel:  out_s = Mee xin_s + scale * (Dhop in)_s  with |out|^2 (EPI_FINAL).
+// Mee = bee - cee Q is bidiagonal in s (reading C5): P+ components take xin_{s-1}, P- components xin_{s+1}, with the
+// -mf wall; the hopping term enters pointwise, so nothing but the slice being written has to stay on chip.
+// (The column-global operators -- Mee^-1 and the A^dag that follows a daggered Dhop -- stay in the column kernels of
+// dwf_fived.cu: an Ls column of one tile does not fit in registers or shared memory next to the staging ring, and a
+// round trip through a global scratch tile costs a DRAM write-back on this L2.)
 struct EpiArgs {
-    int mode;              // EPI_*
-    const void* xin;       // EPI_FINAL / EPI_CG: the field Mee acts on (output parity)
-    void* r;               // EPI_CG: residual, updated in place
-    const double* sc;      // device scalars
-    int slot_c, slot_d;    // EPI_CG: alpha = sc[slot_c] / sc[slot_d]
-    double* partials;      // per-CTA partial sums of |out|^2 (EPI_FINAL) or |r|^2 (EPI_CG); null: none
-    double b5, c5, bee, mcee, mf, scale;     // A = b5 + c5 S ; Mee = bee + mcee S
-    double inva, rho, g0;                    // (bee + mcee S)^-1: 1/bee, cee/bee, 1/(1 + mf rho^Ls)
-    double cj[16];                           // mf rho^{j+1}
+    int mode;              // EPI_NONE or EPI_FINAL
+    const void* xin;       // the field Mee acts on (output parity)
+    double* partials;      // per-CTA partial sums of |out|^2; null: none
+    double bee, mcee, mf, scale;     // Mee = bee + mcee Q
 };
 
 __device__ __forceinline__ float4 vmul(float a, const float4& x) { return make_float4(a * x.x, a * x.y, a * x.z, a * x.w); }
@@ -420,26 +430,6 @@ __device__ __forceinline__ double vnorm2(const double2& a) { return a.x * a.x + 
 __device__ __forceinline__ float4 ldcs_v(const float4* p) { return __ldcs(p); }
 __device__ __forceinline__ double2 ldcs_v(const double2* p) { return __ldcs(p); }
 
-// y = (a + b S)^-1 x in place, x in sweep order
-template <typename R, typename V, int LS>
-__device__ __forceinline__ void col_inv(V (&x)[LS], R inva, R rho, R g0, const R (&cj)[LS]) {
-    x[0] = vmul(inva, x[0]);
-#pragma unroll
-    for (int j = 1; j < LS; ++j) x[j] = vfma(rho, x[j - 1], vmul(inva, x[j]));
-    const V G = vmul(g0, x[LS - 1]);
-#pragma unroll
-    for (int j = 0; j < LS - 1; ++j) x[j] = vfma(-cj[j], G, x[j]);
-    x[LS - 1] = G;
-}
-// y = (a + b S) x in place (descending so that x_{j-1} is still the input)
-template <typename R, typename V, int LS>
-__device__ __forceinline__ void col_bidiag(V (&x)[LS], R a, R b, R mf) {
-    const V wall = vmul(-mf * b, x[LS - 1]);
-#pragma unroll
-    for (int j = LS - 1; j >= 1; --j) x[j] = vfma(b, x[j - 1], vmul(a, x[j]));
-    x[0] = vfma(a, x[0], wall);
-}
-
 struct TmaArgs {
     Geom g;
     const void* in;
@@ -451,99 +441,13 @@ struct TmaArgs {
     int* counters;            // [3] queue / done / round-arrival counters
     EpiArgs epi;
     int l2hint;
+    int skip;                 // debug: bit r set = do not load halo region r (4..11); results are then wrong, traffic only
     int mode;                 // 0: static round-robin, 1: global in-order queue, 2: static rounds, producers in lockstep
     int dagger;
 };
 
 
-// the epilogue of one tile for one consumer thread: its 6 vectors per slice (fp32: all of its site's; fp64: the chirality
-// half it holds), column by column
-template <typename R, int TPS, int LS>
-__device__ __forceinline__ void epilogue(const TmaArgs& a, typename VT<R>::V* __restrict__ outp, int tile, int site, int sub,
-                                         double& nrm) {
-    using V = typename VT<R>::V;
-    constexpr int K = VT<R>::K;
-    constexpr size_t STR = (size_t)K * TSV;          // s stride of a column, in vectors
-    const EpiArgs& e = a.epi;
-    const bool dag = a.dagger != 0;
-    const int k0 = (TPS == 1) ? 0 : sub * 6;
-    const R b5 = (R)e.b5, c5 = (R)e.c5, mf = (R)e.mf;
-    if (e.mode == EPI_MID) {
-        R cj[LS];
-#pragma unroll
-        for (int j = 0; j < LS; ++j) cj[j] = (R)e.cj[j];
-        const R inva = (R)e.inva, rho = (R)e.rho, g0 = (R)e.g0;
-#pragma unroll
-        for (int kb = 0; kb < 6; kb += 2) {
-            V col[2][LS];
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                const bool minus = (TPS == 1) ? (kb + q >= 3) : (sub != 0);
-                const bool rev = minus != dag;
-                V* cp = outp + (size_t)(k0 + kb + q) * TSV;
-#pragma unroll
-                for (int j = 0; j < LS; ++j) col[q][j] = cp[(size_t)(rev ? LS - 1 - j : j) * STR];
-            }
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                if (!dag) { col_inv<R, V, LS>(col[q], inva, rho, g0, cj); col_bidiag<R, V, LS>(col[q], b5, c5, mf); }
-                else      { col_bidiag<R, V, LS>(col[q], b5, c5, mf); col_inv<R, V, LS>(col[q], inva, rho, g0, cj); }
-            }
-#pragma unroll
-            for (int q = 0; q < 2; ++q) {
-                const bool minus = (TPS == 1) ? (kb + q >= 3) : (sub != 0);
-                const bool rev = minus != dag;
-                V* cp = outp + (size_t)(k0 + kb + q) * TSV;
-#pragma unroll
-                for (int j = 0; j < LS; ++j) stcs_v(cp + (size_t)(rev ? LS - 1 - j : j) * STR, col[q][j]);
-            }
-        }
-        return;
-    }
-    // EPI_FINAL / EPI_CG
-    const R bee = (R)e.bee, mcee = (R)e.mcee, scale = (R)e.scale;
-    const size_t toff = (size_t)tile * LS * STR + site;
-    const V* __restrict__ xin = reinterpret_cast<const V*>(e.xin) + toff;
-    V* __restrict__ rres = reinterpret_cast<V*>(e.r) + toff;
-    R alpha = (R)0;
-    if (e.mode == EPI_CG) alpha = (R)(e.sc[e.slot_c] / e.sc[e.slot_d]);
-#pragma unroll
-    for (int kk = 0; kk < 6; ++kk) {
-        const bool minus = (TPS == 1) ? (kk >= 3) : (sub != 0);
-        const bool rev = minus != dag;
-        V* cp = outp + (size_t)(k0 + kk) * TSV;
-        const V* xp = xin + (size_t)(k0 + kk) * TSV;
-        V d[LS], x[LS];
-#pragma unroll
-        for (int j = 0; j < LS; ++j) {
-            const size_t o = (size_t)(rev ? LS - 1 - j : j) * STR;
-            d[j] = cp[o];
-            x[j] = ldcs_v(xp + o);
-        }
-        if (dag) col_bidiag<R, V, LS>(d, b5, c5, mf);      // A^dag on the hopping term
-        col_bidiag<R, V, LS>(x, bee, mcee, mf);             // Mee (Mee^dag) on the diagonal term
-        if (e.mode == EPI_FINAL) {
-#pragma unroll
-            for (int j = 0; j < LS; ++j) {
-                const V o = vfma(scale, d[j], x[j]);
-                nrm += vnorm2(o);
-                stcs_v(cp + (size_t)(rev ? LS - 1 - j : j) * STR, o);
-            }
-        } else {
-            V* rp = rres + (size_t)(k0 + kk) * TSV;
-#pragma unroll
-            for (int j = 0; j < LS; ++j) {
-                const size_t o = (size_t)(rev ? LS - 1 - j : j) * STR;
-                const V z = vfma(scale, d[j], x[j]);
-                const V rn = vfma(-alpha, z, rp[o]);
-                nrm += vnorm2(rn);
-                rp[o] = rn;
-            }
-        }
-    }
-}
-
-template <typename R, int TPS, int NG, int NST, int MINB, int LS>
+template <typename R, int TPS, int NG, int NST, int MINB, int EPI>
 __global__ void __launch_bounds__(128 + 128 * TPS, MINB)
 dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, const __grid_constant__ CUtensorMap map_z,
                 const __grid_constant__ CUtensorMap map_y) {
@@ -626,11 +530,7 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                 nc[mu] = (tc[mu] == 0) ? g.NT[mu] - 1 : tc[mu] - 1;
                 nt[2 * mu + 1] = tile_index(g, nc);
             }
-            if (lane == 0) {
-                next_of[j & 3] = tile_next;       // published by the release-arrive on slice 0's `full` barrier
-                if (tile_next >= 0)               // next tile's links -> L2
-                    l2_prefetch_bulk(reinterpret_cast<const V*>(a.W) + (size_t)tile_next * 8 * KG * TSV, 8 * KG * TSV * 16);
-            }
+            if (lane == 0) next_of[j & 3] = tile_next;       // published by the release-arrive on slice 0's `full` barrier
             ++j;
             const V* src_p = in + (size_t)nt[0] * tile_vecs + xs_p;
             const V* src_m = in + (size_t)nt[1] * tile_vecs + xs_m;
@@ -640,24 +540,29 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                 const uint32_t base = stage0 + st * STAGE_BYTES;
                 mbar_wait(empty, ph ^ 1);
                 if (lane == 0) {
-                    mbar_arrive_expect_tx(full, 10 * REGION_BYTES);
+                    // next tile's links -> L2, issued with this tile's last slice: the consumers want them NST slices
+                    // later (issued a whole tile ahead they were evicted again before use and fetched twice)
+                    if (s == Ls - 1 && tile_next >= 0)
+                        l2_prefetch_bulk(reinterpret_cast<const V*>(a.W) + (size_t)tile_next * 8 * KG * TSV, 8 * KG * TSV * 16);
+                    const int nskip = __popc(a.skip & 0x3f0);
+                    mbar_arrive_expect_tx(full, (10 - nskip) * REGION_BYTES);
                     const int row_own = (tile * Ls + s) * K;
 #pragma unroll
                     for (int tt = 0; tt < 4; ++tt) tma_load_3d_hint(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full, pol);
-                    tma_load_3d_hint(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full, pol);
-                    tma_load_3d_hint(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full, pol);
-                    tma_load_4d_hint(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full, pol);
-                    tma_load_4d_hint(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full, pol);
-                    tma_load_4d_hint(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full, pol);
-                    tma_load_4d_hint(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full, pol);
+                    if (!(a.skip & 0x010)) tma_load_3d_hint(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full, pol);
+                    if (!(a.skip & 0x020)) tma_load_3d_hint(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full, pol);
+                    if (!(a.skip & 0x040)) tma_load_4d_hint(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full, pol);
+                    if (!(a.skip & 0x080)) tma_load_4d_hint(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full, pol);
+                    if (!(a.skip & 0x100)) tma_load_4d_hint(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full, pol);
+                    if (!(a.skip & 0x200)) tma_load_4d_hint(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full, pol);
                 }
                 const V* sp = src_p + (size_t)s * (K * TSV);
                 const V* sm = src_m + (size_t)s * (K * TSV);
                 const uint32_t dp = base + 10 * REGION_BYTES + lane * 16, dm = base + 11 * REGION_BYTES + lane * 16;
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-                    cp_async16_hint(dp + k * 512, sp + k * TSV, pol);
-                    cp_async16_hint(dm + k * 512, sm + k * TSV, pol);
+                    if (!(a.skip & 0x400)) cp_async16_hint(dp + k * 512, sp + k * TSV, pol);
+                    if (!(a.skip & 0x800)) cp_async16_hint(dm + k * 512, sm + k * TSV, pol);
                 }
                 cp_async_mbar_arrive_noinc(full);
             }
@@ -719,11 +624,27 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
             }
         }
         V* __restrict__ outp = reinterpret_cast<V*>(a.out) + (size_t)tile * Ls * K * TSV + site;
+        const V* __restrict__ xin_t = reinterpret_cast<const V*>(a.epi.xin) + (size_t)tile * Ls * K * TSV + site;
         for (int s = 0; s < Ls; ++s, ++n) {
             const uint32_t st = n % NST, ph = (n / NST) & 1;
             const uint32_t base = stage0 + st * STAGE_BYTES;
             mbar_wait(bar0 + 8 * st, ph);
             if (s == 0) tile_next = *(volatile int*)&next_of[j & 3];
+            if constexpr (EPI != 0) {
+                // the epilogue's xin rows -> L2 one slice ahead (slice 0 also fetches itself and the wall slice)
+                const V* xk = xin_t + ((TPS == 1) ? 0 : sub * (K / 2)) * TSV;
+                if (s + 1 < Ls) {
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) l2_prefetch(xk + (size_t)(s + 1) * (K * TSV) + k * TSV);
+                }
+                if (s == 0) {
+#pragma unroll
+                    for (int k = 0; k < 6; ++k) {
+                        l2_prefetch(xk + k * TSV);
+                        l2_prefetch(xk + (size_t)(Ls - 1) * (K * TSV) + k * TSV);
+                    }
+                }
+            }
             R acc[24];
 #pragma unroll
             for (int j = 0; j < LPT; ++j) {
@@ -743,11 +664,23 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
             __syncwarp();
             if (lane == 0) mbar_arrive(bar0 + 8 * (NST + st));      // stage released
             V* o = outp + (size_t)s * (K * TSV);
-            const bool keep = (LS > 0) && a.epi.mode != EPI_NONE;      // the epilogue re-reads the tile from L2
+            // EPI: out_s = bee xin_s + mcee (Q xin)_s + scale D_s, |out|^2 summed (Mee xin - 1/4 Dhop ..., reading C6)
+            const R e_bee = (R)a.epi.bee, e_scale = (R)a.epi.scale;
+            const R e_wm = (R)((s > 0) ? a.epi.mcee : -a.epi.mf * a.epi.mcee);            // P+ : xin_{s-1}
+            const R e_wp = (R)((s + 1 < Ls) ? a.epi.mcee : -a.epi.mf * a.epi.mcee);       // P- : xin_{s+1}
+            const V* xs = xin_t + (size_t)s * (K * TSV);
+            const V* xm = xin_t + (size_t)((s > 0) ? s - 1 : Ls - 1) * (K * TSV);
+            const V* xp = xin_t + (size_t)((s + 1 < Ls) ? s + 1 : 0) * (K * TSV);
             if (TPS == 1) {
-                if (keep) {
+                if constexpr (EPI != 0) {
 #pragma unroll
-                    for (int k = 0; k < K; ++k) o[k * TSV] = packv(acc + k * VW);
+                    for (int k = 0; k < K; ++k) {
+                        const V xc = ldg_v(xs + k * TSV);
+                        const V xn = ldg_v(((k < K / 2) ? xm : xp) + k * TSV);
+                        const V ov = vfma(e_scale, packv(acc + k * VW), vfma((k < K / 2) ? e_wm : e_wp, xn, vmul(e_bee, xc)));
+                        nrm += vnorm2(ov);
+                        stcs_v(o + k * TSV, ov);
+                    }
                 } else {
 #pragma unroll
                     for (int k = 0; k < K; ++k) stcs_v(o + k * TSV, packv(acc + k * VW));
@@ -761,23 +694,28 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                     const R keep = sub ? acc[12 + i] : acc[i];
                     mine[i] = keep + shfl16(send);
                 }
-                V* o2 = o + (sub ? (K / 2) * TSV : 0);
-                if (keep) {
+                const int k0 = sub ? (K / 2) : 0;
+                V* o2 = o + k0 * TSV;
+                if constexpr (EPI != 0) {
+                    const V* xc_p = xs + k0 * TSV;
+                    const V* xn_p = (sub ? xp : xm) + k0 * TSV;
+                    const R w = sub ? e_wp : e_wm;
 #pragma unroll
-                    for (int k = 0; k < K / 2; ++k) o2[k * TSV] = packv(mine + k * VW);
+                    for (int k = 0; k < K / 2; ++k) {
+                        const V ov = vfma(e_scale, packv(mine + k * VW), vfma(w, ldg_v(xn_p + k * TSV), vmul(e_bee, ldg_v(xc_p + k * TSV))));
+                        nrm += vnorm2(ov);
+                        stcs_v(o2 + k * TSV, ov);
+                    }
                 } else {
 #pragma unroll
                     for (int k = 0; k < K / 2; ++k) stcs_v(o2 + k * TSV, packv(mine + k * VW));
                 }
             }
         }
-        if constexpr (LS > 0) {
-            if (a.epi.mode != EPI_NONE) epilogue<R, TPS, LS>(a, outp, tile, site, sub, nrm);
-        }
         tile = tile_next;
         ++j;
     }
-    if (LS > 0 && a.epi.mode >= EPI_FINAL && a.epi.partials != nullptr) {
+    if (EPI != 0 && a.epi.partials != nullptr) {
         // fixed-tree sum over the consumer threads (static tile assignment: bit-reproducible run to run)
         __shared__ double wsum[NCW];
 #pragma unroll
@@ -794,11 +732,11 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
 }
 
 // ------------------------------------------------------------------------------------------ launch
-template <typename R, int TPS, int NG, int NST, int MINB, int LS>
+template <typename R, int TPS, int NG, int NST, int MINB, int EPI>
 static dwf_status launch_tma_t(dwf_ctx* c, const TmaArgs& a, const CUtensorMap* maps, int* grid_out) {
     constexpr int K = VT<R>::K;
     const size_t smem = (size_t)NST * NREG * K * 512;
-    auto kern = dhop_tma_kernel<R, TPS, NG, NST, MINB, LS>;
+    auto kern = dhop_tma_kernel<R, TPS, NG, NST, MINB, EPI>;
     static bool attr_done = false;
     if (!attr_done) {
         DWF_CUDA_CHECK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -829,6 +767,7 @@ static dwf_status fill_args(dwf_ctx* c, TmaArgs& a, void* out, const void* in, i
     a.counters = s->counters;
     a.mode = c->dhop_dynamic;
     a.l2hint = c->dhop_l2hint;
+    a.skip = c->dhop_skip;
     a.dagger = dagger;
     a.epi.mode = EPI_NONE;
     return DWF_OK;
@@ -849,50 +788,39 @@ dwf_status launch_dhop_tma(dwf_ctx* c, void* out, const void* in, int out_parity
                          : launch_tma_t<float, 1, 18, 3, 2, 0>(c, a, maps, nullptr);
 }
 
-// the fused kernels exist for 4^4 tiles, 2-row links and Ls = 8, 12, 16 (the Ls column lives in registers)
-bool dhop_fused_available(const dwf_ctx* c) {
-    return c->tma != nullptr && c->fuse && c->compress12 && (c->g.Ls == 8 || c->g.Ls == 12 || c->g.Ls == 16);
-}
+// the fused kernel exists for 4^4 tiles with 2-row links (any Ls)
+bool dhop_fused_available(const dwf_ctx* c) { return c->tma != nullptr && c->fuse && c->compress12; }
 
-dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, int epi,
-                             const void* xin, double scale, void* r, int slot_c, int slot_d, int norm_slot) {
+// out = Mee xin + scale Dhop in (non-daggered), norm_slot >= 0: |out|^2 -> scalars[norm_slot]
+dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_parity, int prec, const void* xin, double scale,
+                             int norm_slot) {
     if (!dhop_fused_available(c)) { c->err = "fused Dhop kernel not available for this geometry"; return DWF_ESTATE; }
     const CUtensorMap* maps = nullptr;
     TmaArgs a;
-    dwf_status st = fill_args(c, a, out, in, out_parity, dagger, prec, &maps);
+    dwf_status st = fill_args(c, a, out, in, out_parity, 0, prec, &maps);
     if (st != DWF_OK) return st;
-    const int Ls = c->g.Ls;
     const double bee = 1.0 + c->b5 * (4.0 - c->M5), cee = 1.0 - c->c5 * (4.0 - c->M5);
     EpiArgs& e = a.epi;
-    e.mode = epi;
-    e.xin = xin; e.r = r; e.sc = c->scalars; e.slot_c = slot_c; e.slot_d = slot_d;
-    e.b5 = c->b5; e.c5 = c->c5; e.bee = bee; e.mcee = -cee; e.mf = c->mf; e.scale = scale;
-    e.inva = 1.0 / bee; e.rho = cee / bee; e.g0 = 1.0 / (1.0 + c->mf * std::pow(e.rho, Ls));
-    for (int j = 0; j < 16; ++j) e.cj[j] = (j < Ls) ? c->mf * std::pow(e.rho, j + 1) : 0.0;
+    e.mode = EPI_FINAL;
+    e.xin = xin;
+    e.bee = bee; e.mcee = -cee; e.mf = c->mf; e.scale = scale;
     a.mode = 0;                                    // static tile assignment: reproducible reductions
     int grid = 0;
-    st = dhop_time_begin(c);
-    if (st != DWF_OK) return st;
     if (norm_slot >= 0) {
         TmaState* s = (TmaState*)c->tma;
-        st = ensure_partials(c, s->num_sms * 2);
+        st = ensure_partials(c, std::max(s->num_sms * 2, c->dhop_grid));
         if (st != DWF_OK) return st;
         e.partials = c->partials;
     }
-#define DWF_FUSED(LSV)                                                                                     \
-    st = (prec == DWF_F64) ? launch_tma_t<double, 2, 12, 3, 1, LSV>(c, a, maps, &grid)                     \
-                           : launch_tma_t<float, 1, 12, 3, 2, LSV>(c, a, maps, &grid)
-    if (Ls == 8) DWF_FUSED(8);
-    else if (Ls == 12) DWF_FUSED(12);
-    else DWF_FUSED(16);
-#undef DWF_FUSED
+    st = dhop_time_begin(c);
     if (st != DWF_OK) return st;
-    {   // algorithmic bytes: the input field, the links, the extra epilogue operands, one field written
-        const double S = (double)half_bytes(c->g, prec), B = (prec == DWF_F64) ? 8.0 : 4.0;
-        const double nfields = (epi == EPI_MID) ? 2.0 : (epi == EPI_FINAL ? 3.0 : 4.0);
-        st = dhop_time_end(c, nfields * S + (double)c->g.Vh * 8 * 12 * B);
-        if (st != DWF_OK) return st;
-    }
+    st = (prec == DWF_F64) ? launch_tma_t<double, 2, 12, 3, 1, 1>(c, a, maps, &grid)
+                           : launch_tma_t<float, 1, 12, 3, 2, 1>(c, a, maps, &grid);
+    if (st != DWF_OK) return st;
+    // algorithmic bytes: the input field, xin, the links, one field written
+    const double B = (prec == DWF_F64) ? 8.0 : 4.0;
+    st = dhop_time_end(c, 3.0 * (double)half_bytes(c->g, prec) + (double)c->g.Vh * 8 * 12 * B);
+    if (st != DWF_OK) return st;
     if (norm_slot >= 0) return launch_reduce(c, grid, norm_slot);
     return DWF_OK;
 }

@@ -328,3 +328,75 @@ dwf_status launch_op5(dwf_ctx* c, void* out, const void* x, int op1, const void*
 }
 
 }  // namespace dwf
+
+namespace dwf {
+// CG residual step (reading C8: r -= alpha Mpc^dag q) in one streaming column kernel.  The last step of Mpc^dag,
+// z = Mee^dag q - 1/4 A^dag d, is bidiagonal in s on both operands (reading C5): in sweep order (daggered operators:
+// s descending on P+ components, ascending on P-) (Q^dag x)_j is the previous element, the -mf wall at j = 0, so
+//     z_j = bee q_j - cee q_{j-1} + yscale (b5 d_j + c5 d_{j-1})
+// is formed in registers and never stored; r -= alpha z with alpha = sc[slot_c]/sc[slot_d]; |r|^2 -> partials.
+template <typename R>
+__global__ void __launch_bounds__(128) cg_r_kernel(int Ls, int TS, unsigned nvec_site, typename V5<R>::V* __restrict__ r,
+                                                   const typename V5<R>::V* __restrict__ q,
+                                                   const typename V5<R>::V* __restrict__ d, const double* __restrict__ sc,
+                                                   int slot_c, int slot_d, R bee, R mcee, R yb5, R yc5, R mf,
+                                                   double* __restrict__ partials) {
+    using V = typename V5<R>::V;
+    constexpr int K = V5<R>::K;
+    const unsigned gid = blockIdx.x * blockDim.x + threadIdx.x;
+    double nrm = 0.0;
+    if (gid < nvec_site) {
+        const unsigned per_tile = (unsigned)K * TS;
+        const unsigned tile = gid / per_tile, j = gid - tile * per_tile;
+        const int k = j / TS;
+        const bool rev = (k < K / 2);          // daggered: P+ components walk s downwards
+        const size_t base = (size_t)tile * Ls * per_tile + j;
+        const R alpha = (R)(sc[slot_c] / sc[slot_d]);
+        const size_t olast = base + (size_t)(rev ? 0 : Ls - 1) * per_tile;
+        V qprev = q[olast], dprev = d[olast];
+        scalev(qprev, -mf);
+        scalev(dprev, -mf);
+#pragma unroll 4
+        for (int jj = 0; jj < Ls; ++jj) {
+            const size_t o = base + (size_t)(rev ? Ls - 1 - jj : jj) * per_tile;
+            const V qv = q[o], dv = d[o];
+            V z = zerov((V*)nullptr);
+            fmav(z, bee, qv);
+            fmav(z, mcee, qprev);
+            fmav(z, yb5, dv);
+            fmav(z, yc5, dprev);
+            V rv = r[o];
+            fmav(rv, -alpha, z);
+            r[o] = rv;
+            nrm += norm2v(rv);
+            qprev = qv;
+            dprev = dv;
+        }
+    }
+    const double tot = block_reduce_sum(nrm);
+    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+}
+
+dwf_status launch_cg_r(dwf_ctx* c, void* r, const void* q, const void* d, double yscale, int prec, int slot_c, int slot_d,
+                       int norm_slot) {
+    const Geom& g = c->g;
+    const double bee = 1.0 + c->b5 * (4.0 - c->M5), cee = 1.0 - c->c5 * (4.0 - c->M5);
+    const int block = 128;
+    const unsigned nvec_site = (unsigned)g.Vh * (prec == DWF_F64 ? 12 : 6);
+    const int grid = (int)((nvec_site + block - 1) / block);
+    dwf_status st = ensure_partials(c, grid);
+    if (st != DWF_OK) return st;
+    if (prec == DWF_F64)
+        cg_r_kernel<double><<<grid, block, 0, c->stream>>>(g.Ls, g.TS, nvec_site, (double2*)r, (const double2*)q,
+                                                           (const double2*)d, c->scalars, slot_c, slot_d, bee, -cee,
+                                                           yscale * c->b5, yscale * c->c5, c->mf, c->partials);
+    else
+        cg_r_kernel<float><<<grid, block, 0, c->stream>>>(g.Ls, g.TS, nvec_site, (float4*)r, (const float4*)q,
+                                                          (const float4*)d, c->scalars, slot_c, slot_d, (float)bee,
+                                                          (float)-cee, (float)(yscale * c->b5), (float)(yscale * c->c5),
+                                                          (float)c->mf, c->partials);
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return launch_reduce(c, grid, norm_slot);
+}
+}  // namespace dwf

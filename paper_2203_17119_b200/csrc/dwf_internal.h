@@ -60,6 +60,7 @@ struct dwf_ctx {
     int dhop_grid = 0;     // CTAs of the persistent TMA kernel (0 = SMs x resident CTAs)
     int fuse = 1;          // Mpc / CG through the Dhop kernel's fused 5-D epilogues when the TMA kernel applies (0: separate op5 kernels)
     int dhop_dynamic = 0;  // TMA kernel tile scheduling: 0 static round-robin, 1 global in-order queue, 2 static rounds in lockstep
+    int dhop_skip = 0;     // debug only (traffic attribution): halo regions the TMA kernel does not load
     int dhop_l2hint = 0;   // L2 eviction priority of the TMA kernel's input-field reads: 0 normal, 1 evict_last, 2 evict_first
     int dhop_order = 0;    // tile traversal of the TMA kernel: blob extents in tiles as digits (0 = default), dwf_dhop_tma.cu
     int dhop_order_axes = 0;   // blob path, fastest-first axis digits
@@ -139,14 +140,14 @@ dwf_status launch_dhop_pipe(dwf_ctx* c, void* out, const void* in, int out_parit
 dwf_status tma_state_build(dwf_ctx* c);
 void tma_state_free(dwf_ctx* c);
 dwf_status launch_dhop_tma(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, bool* handled);
-// Dhop with a fused 5-D epilogue on the output columns (dwf_dhop_tma.cu):
-//   EPI_MID   : out = A Mee^-1 Dhop in            (dagger: Mee^-dag A^dag Dhop^dag in)
-//   EPI_FINAL : out = Mee xin + scale Dhop in     (dagger: Mee^dag xin + scale A^dag Dhop^dag in); norm_slot >= 0: |out|^2
-//   EPI_CG    : z as EPI_FINAL(dagger), r -= (sc[slot_c]/sc[slot_d]) z, |r|^2 -> norm_slot; out is scratch
-enum { EPI_NONE = 0, EPI_MID = 1, EPI_FINAL = 2, EPI_CG = 3 };
+// Dhop with the fused last step of Mpc (dwf_dhop_tma.cu): out = Mee xin + scale Dhop in, norm_slot >= 0: |out|^2
+enum { EPI_NONE = 0, EPI_FINAL = 1 };
 bool dhop_fused_available(const dwf_ctx* c);
-dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, int epi,
-                             const void* xin, double scale, void* r, int slot_c, int slot_d, int norm_slot);
+dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_parity, int prec, const void* xin, double scale,
+                             int norm_slot);
+// r -= (sc[slot_c]/sc[slot_d]) (Mee^dag q + yscale A^dag d); |r|^2 -> scalars[norm_slot]   (dwf_fived.cu)
+dwf_status launch_cg_r(dwf_ctx* c, void* r, const void* q, const void* d, double yscale, int prec, int slot_c, int slot_d,
+                       int norm_slot);
 // x += a p (a = sc[slot_c]/sc[slot_d]); p = r + b p (b = sc[slot_cn]/sc[slot_c]); ap = A p.  init: p = r, ap = A p only.
 dwf_status launch_cg_xp(dwf_ctx* c, void* x, void* p, const void* r, void* ap, int prec, int slot_c, int slot_d,
                         int slot_cn, int init);
