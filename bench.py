@@ -206,7 +206,7 @@ def run_dwf(args, cfg):
     e.record()
     barrier()
     ms = s.elapsed_time(e)
-    dhop_ms, dhop_n = g.get_option("dhop_ms"), g.get_option("dhop_timed")
+    dhop_ms, dhop_n, dhop_bytes_total = g.get_option("dhop_ms"), g.get_option("dhop_timed"), g.get_option("dhop_bytes")
     launches = g.launch_count() - l0
     g.set_option("time_dhop", 0)
     clocks = sampler.stop()
@@ -217,17 +217,18 @@ def run_dwf(args, cfg):
     ms_step = ms / args.steps
     value = world * segment_flops(n5h, iters) / (ms_step * 1e-3) / 1e9
 
-    # ---- roofline of the dominant kernel: half-volume fp64 Dhop
-    ng = 12
-    dhop_bytes = n5h * 48 * 8 + (cfg.V4 // 2) * 8 * ng * 8
+    # ---- roofline of the dominant kernel: the half-volume fp64 Dhop kernel.  Per launch the library
+    # sums the ALGORITHMIC bytes (field in + field out + 12-real links, + the Mee operand for the launch that carries
+    # the fused epilogue) next to the event pair it records on its stream.
     dhop_avg_ms = dhop_ms / max(dhop_n, 1)
+    dhop_bytes = dhop_bytes_total / max(dhop_n, 1)
     achieved = dhop_bytes / (dhop_avg_ms * 1e-3) / 1e9
     traffic = None
     tp = os.path.join(ROOT, "profiles", "dhop_traffic.json")
     if os.path.exists(tp):
         traffic = json.load(open(tp)).get("dhop_f64_dram_bytes_per_launch")
-    roofline = {"bound": "hbm", "kernel": "dhop_kernel<double> (half-volume, 12-real links)", "achieved": achieved,
-                "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / hbm_peak,
+    roofline = {"bound": "hbm", "kernel": "dhop_tma_kernel<double> (half-volume, 12-real links; per CG iteration 3 plain launches + 1 with the fused Mee epilogue)",
+                "achieved": achieved, "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / hbm_peak,
                 "traffic": traffic, "algorithmic_bytes_per_launch": dhop_bytes, "avg_launch_ms": dhop_avg_ms,
                 "launches_timed": int(dhop_n), "share_of_step": dhop_ms / ms if ms > 0 else None,
                 "gflops": FLOP_DHOP * n5h / (dhop_avg_ms * 1e-3) / 1e9}

@@ -1,0 +1,84 @@
+"""GPU parity at BASELINE.json's full size, in the launch configuration bench.py times: configs[3] = c4,
+32^4 x Ls=12 Moebius, 2-row compressed links, the seeded eps = 0.7 gauge field and Gaussian source of bench.py.
+
+The oracle finishes one operator application at this size in seconds, so the comparison is element by element on the
+WHOLE field (stricter than sampled outputs): Dhop in fp64 and fp32, Mpc, Mpc^dag Mpc, and the first iterations of the
+red-black CG (recurrence-residual history, then the oracle recomputes the true residual of the GPU iterate)."""
+import numpy as np
+import pytest
+
+from paper_2203_17119_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+def rel(a, b):
+    a = np.asarray(a, dtype=np.complex128).ravel()
+    b = np.asarray(b, dtype=np.complex128).ravel()
+    return float(np.linalg.norm(a - b) / np.linalg.norm(b))
+
+
+@pytest.fixture(scope="module")
+def c4(oracle_built):
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2203_17119_b200 import api
+    from oracle.dwf_oracle import Oracle
+    cfg = inputs.CONFIGS["c4"]
+    U = inputs.make_gauge(cfg)
+    g = api.from_config(cfg, device="cuda:0")
+    g.set_gauge(U)
+    orc = Oracle(cfg.dims, cfg.Ls, cfg.M5, cfg.mf, cfg.b5, cfg.c5, antiperiodic_t=cfg.antiperiodic_t, cut=cfg.cut).set_gauge(U)
+    odd = inputs.source_half(cfg.dims, cfg.Ls, cfg.source_seed, parity=1)
+    yield dict(api=api, cfg=cfg, g=g, orc=orc, odd=odd, U=U)
+    g.close()
+
+
+def test_c4_runs_the_fast_kernels(c4):
+    g = c4["g"]
+    assert [int(g.get_option(f"tile_{k}")) for k in "xyzt"] == [4, 4, 4, 4]
+    assert g.get_option("compress12") == 1 and g.get_option("fused_active") == 1
+
+
+def test_c4_dhop_fp64_full_field(c4):
+    A, g, orc, odd = c4["api"], c4["g"], c4["orc"], c4["odd"]
+    got = g.unpack(g.dhop(g.pack(odd, A.F64, A.ODD), A.EVEN, False, A.F64), A.F64, A.EVEN)
+    assert rel(got, orc.dhop(odd, 0, False)) < 1e-12
+    got = g.unpack(g.dhop(g.pack(odd, A.F64, A.ODD), A.EVEN, True, A.F64), A.F64, A.EVEN)
+    assert rel(got, orc.dhop(odd, 0, True)) < 1e-12
+
+
+def test_c4_dhop_fp32_full_field(c4):
+    from oracle.dwf_oracle import Oracle
+    A, g, cfg, odd = c4["api"], c4["g"], c4["cfg"], c4["odd"]
+    U32 = c4["U"].astype(np.complex64).astype(np.complex128)
+    orc32 = Oracle(cfg.dims, cfg.Ls, cfg.M5, cfg.mf, cfg.b5, cfg.c5, antiperiodic_t=cfg.antiperiodic_t, cut=cfg.cut).set_gauge(U32)
+    src = odd.astype(np.complex64).astype(np.complex128)
+    got = g.unpack(g.dhop(g.pack(src, A.F32, A.ODD), A.EVEN, False, A.F32), A.F32, A.EVEN)
+    assert rel(got, orc32.dhop(src, 0, False)) < 1e-5
+
+
+def test_c4_mpc_and_mdagm_full_field(c4):
+    A, g, orc, odd = c4["api"], c4["g"], c4["orc"], c4["odd"]
+    nat = g.pack(odd, A.F64, A.ODD)
+    assert rel(g.unpack(g.mpc(nat, False, A.F64), A.F64, A.ODD), orc.mpc(odd)) < 1e-12
+    assert rel(g.unpack(g.mpc(nat, True, A.F64), A.F64, A.ODD), orc.mpc(odd, dagger=True)) < 1e-12
+    assert rel(g.unpack(g.mdagm(nat, A.F64), A.F64, A.ODD), orc.mdagm(odd)) < 2e-12
+
+
+def test_c4_cg_first_iterations_match_oracle(c4):
+    """A full oracle CG at this size costs ~10 s per iteration x 254 iterations; reading of SURVEY 8(d): residual-history
+    agreement over the first K iterations, then the oracle recomputes the true residual of the GPU iterate."""
+    from oracle.dwf_oracle import cg
+    A, g, orc, odd = c4["api"], c4["g"], c4["orc"], c4["odd"]
+    K = 4
+    hist = []
+    cg(orc, odd, 1e-30, K, history=hist, restart_on_true=False)
+    nat = g.pack(odd, A.F64, A.ODD)
+    for k in range(1, K + 1):
+        x, info, st = g.cg(nat, 1e-30, k, A.CG_F64)
+        assert st == A.ENOTCONV and info["iters_total"] == k
+        assert abs(info["resid_iter"] - hist[k - 1]) <= 1e-10 * hist[k - 1], (k, info, hist)
+    xs = g.unpack(x, A.F64, A.ODD)
+    true_res = np.sqrt(orc.norm2(odd - orc.mdagm(xs)) / orc.norm2(odd))
+    assert abs(info["resid_true"] - true_res) <= 1e-9 * true_res
