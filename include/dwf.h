@@ -78,8 +78,15 @@ dwf_status dwf_destroy(dwf_ctx* ctx);
  *   "inner_tol" (default 1e-4), "max_restarts" (default 20)     mixed-precision CG (reading C9), any time
  *   "dhop_sc" s-slices per thread in the Dhop kernel, "dhop_loop_s" 0/1, any time (tuning)
  *   "time_dhop" 0/1: bracket every Dhop kernel launch with CUDA events on the context stream (restarts the
- *   accumulators); dwf_get_option "dhop_ms" / "dhop_timed" then synchronise and return the summed kernel time
- *   and the number of launches timed (bench.py's roofline figure) */
+ *   accumulators); dwf_get_option "dhop_ms" / "dhop_timed" / "dhop_bytes" then synchronise and return the summed
+ *   kernel time, the number of launches timed and their summed algorithmic bytes (bench.py's roofline figure)
+ *   "fuse" 0/1 (default 1), any time: Mpc / CG use the Dhop kernel's fused Mee epilogue and the streaming CG column
+ *   kernels where the TMA Dhop kernel applies (4^4 tiles, 2-row links); get "fused_active" tells whether they do
+ *   "dhop_kernel" 0 auto / 1 shape-generic / 2 cp.async tile kernel, "dhop_grid" CTAs of the persistent TMA kernel,
+ *   "dhop_order" / "dhop_order_axes" tile traversal (blob extents / path axes as decimal digits),
+ *   "dhop_dynamic" 0 static round-robin / 1 global in-order queue / 2 lockstep rounds, "dhop_l2hint" 0/1/2
+ *   (normal / evict_last / evict_first on input reads): tuning, any time.  "dhop_skip" is a measurement aid
+ *   (bit r: halo region r is not loaded; results are then WRONG) and must stay 0 otherwise. */
 dwf_status dwf_set_option(dwf_ctx* ctx, const char* key, double val);
 dwf_status dwf_get_option(const dwf_ctx* ctx, const char* key, double* val);
 /* cudaStream_t as void* (torch.cuda.current_stream().cuda_stream); NULL = default stream */

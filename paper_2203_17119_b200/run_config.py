@@ -1,0 +1,83 @@
+"""Run one BASELINE.json configuration (c1..c5) end to end on the GPU and print one JSON report:
+
+    python -m paper_2203_17119_b200.run_config c5 [--no-uncut]
+
+Seeded synthetic gauge field and source (inputs.py), Dhop / Mpc^dag Mpc timings in fp32 and fp64, then the solve the
+configuration names: red-black CG on Mpc^dag Mpc to cfg.tol in fp64 and in fp32-inner / fp64-outer mixed precision.
+For a configuration with a Dirichlet cut (c2, c5) the same solve is repeated with the uncut operator on the same gauge
+field ("Dirichlet D_Omega solve vs full-operator solve", BASELINE configs[4]; PAPER.md:34 expects the cut operator to
+be the worse conditioned one).  Everything runs in libdwf_b200.so; no oracle, no CPU fallback."""
+from __future__ import annotations
+
+import argparse
+import dataclasses
+import json
+import time
+
+import torch
+
+from . import api, inputs
+
+FLOP_DHOP, FLOP_MPC = 1320, 2 * 1320 + 360
+
+
+def _time(fn, reps):
+    for _ in range(3):
+        fn()
+    s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    s.record()
+    for _ in range(reps):
+        fn()
+    e.record()
+    torch.cuda.synchronize()
+    return s.elapsed_time(e) / reps
+
+
+def run(cfg, U, b_np, with_sweeps=True, max_iter=50000):
+    A = api
+    g = api.from_config(cfg)
+    g.set_gauge(U)
+    n5h = (cfg.V4 // 2) * cfg.Ls
+    rep = {"dims": list(cfg.dims), "Ls": cfg.Ls, "cut": list(cfg.cut), "fused_active": bool(g.get_option("fused_active"))}
+    if with_sweeps:
+        for prec, name in ((A.F32, "f32"), (A.F64, "f64")):
+            src = g.new_native(prec, A.FULL).normal_()
+            dst = g.new_native(prec, A.FULL)
+            ms = _time(lambda: g.dhop(src, A.FULL, False, prec, out=dst), 10)
+            h = src.numel() // 2
+            ms2 = _time(lambda: g.mdagm(src[:h], prec, out=dst[:h]), 5)
+            rep[f"dhop_{name}"] = {"ms_full_volume": ms, "gflops": FLOP_DHOP * 2 * n5h / ms / 1e6}
+            rep[f"mdagm_{name}"] = {"ms": ms2, "gflops": 2 * FLOP_MPC * n5h / ms2 / 1e6}
+            del src, dst
+    b = g.pack(b_np, A.F64, A.ODD)
+    for mode, name in ((A.CG_F64, "cg_f64"), (A.CG_MIXED, "cg_mixed")):
+        x, info, st = g.cg(b, cfg.tol, max_iter, mode)
+        rep[name] = {"tol": cfg.tol, "status": int(st), "iters": info["iters_total"], "restarts": info["restarts"],
+                     "resid_true": info["resid_true"], "seconds": info["seconds"], "launches": info["launches"]}
+        del x
+    g.close()
+    return rep
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("config", choices=sorted(inputs.CONFIGS))
+    ap.add_argument("--no-uncut", action="store_true", help="cut configurations: skip the uncut comparison solve")
+    args = ap.parse_args()
+    if not torch.cuda.is_available():
+        raise SystemExit("run_config needs a CUDA device: the hot path has no CPU fallback")
+    cfg = inputs.CONFIGS[args.config]
+    t0 = time.perf_counter()
+    U = inputs.make_gauge(cfg)
+    b = inputs.source_half(cfg.dims, cfg.Ls, cfg.source_seed, parity=1)
+    out = {"config": cfg.name, "params": {"M5": cfg.M5, "mf": cfg.mf, "b5": cfg.b5, "c5": cfg.c5, "gauge": cfg.gauge, "eps": cfg.eps},
+           "plaquette": inputs.plaquette(U), "input_seconds": time.perf_counter() - t0}
+    out["as_configured"] = run(cfg, U, b)
+    if any(cfg.cut) and not args.no_uncut:
+        out["uncut_operator"] = run(dataclasses.replace(cfg, cut=(0, 0, 0, 0)), U, b, with_sweeps=False)
+    print(json.dumps(out), flush=True)
+
+
+if __name__ == "__main__":
+    main()

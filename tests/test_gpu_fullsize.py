@@ -82,3 +82,42 @@ def test_c4_cg_first_iterations_match_oracle(c4):
     xs = g.unpack(x, A.F64, A.ODD)
     true_res = np.sqrt(orc.norm2(odd - orc.mdagm(xs)) / orc.norm2(odd))
     assert abs(info["resid_true"] - true_res) <= 1e-9 * true_res
+
+
+# ---- BASELINE configs[2] = c3: 24^4 x Ls=16 Moebius, eps = 0.5: Dhop in both precisions, mixed-precision CG to 1e-10
+@pytest.fixture(scope="module")
+def c3(oracle_built):
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2203_17119_b200 import api
+    from oracle.dwf_oracle import Oracle
+    cfg = inputs.CONFIGS["c3"]
+    U = inputs.make_gauge(cfg)
+    g = api.from_config(cfg, device="cuda:0")
+    g.set_gauge(U)
+    orc = Oracle(cfg.dims, cfg.Ls, cfg.M5, cfg.mf, cfg.b5, cfg.c5, antiperiodic_t=cfg.antiperiodic_t, cut=cfg.cut).set_gauge(U)
+    odd = inputs.source_half(cfg.dims, cfg.Ls, cfg.source_seed, parity=1)
+    yield dict(api=api, cfg=cfg, g=g, orc=orc, odd=odd)
+    g.close()
+
+
+def test_c3_dhop_both_precisions_full_field(c3):
+    A, g, orc, odd = c3["api"], c3["g"], c3["orc"], c3["odd"]
+    got = g.unpack(g.dhop(g.pack(odd, A.F64, A.ODD), A.EVEN, False, A.F64), A.F64, A.EVEN)
+    want = orc.dhop(odd, 0, False)
+    assert rel(got, want) < 1e-12
+    # fp32 kernel on the fp32-rounded source; its links are the fp64 links rounded to nearest (reading C10), so the
+    # fp64 oracle on unrounded links differs by the link rounding too: 1e-5 bar of the north star
+    src = odd.astype(np.complex64).astype(np.complex128)
+    got32 = g.unpack(g.dhop(g.pack(src, A.F32, A.ODD), A.EVEN, False, A.F32), A.F32, A.EVEN)
+    assert rel(got32, orc.dhop(src, 0, False)) < 1e-5
+
+
+def test_c3_mixed_precision_cg_to_1e10(c3):
+    A, g, orc, odd, cfg = c3["api"], c3["g"], c3["orc"], c3["odd"], c3["cfg"]
+    x, info, st = g.cg(g.pack(odd, A.F64, A.ODD), cfg.tol, 50000, A.CG_MIXED)
+    assert st == A.OK and info["resid_true"] <= cfg.tol and 1 <= info["restarts"] <= 20
+    xs = g.unpack(x, A.F64, A.ODD)
+    true_res = np.sqrt(orc.norm2(odd - orc.mdagm(xs)) / orc.norm2(odd))      # the oracle recomputes it
+    assert true_res <= cfg.tol * (1 + 1e-6)
+    assert abs(true_res - info["resid_true"]) <= 1e-6 * true_res + 1e-16
