@@ -217,6 +217,56 @@ def cg(orc: Oracle, b, tol, max_iter, x0=None, history=None, restart_on_true=Tru
 
 
 # ---------------------------------------------------------------------------
+# NEXT-2: multishift CG on A + sigma_i, A = Mpc^dag Mpc -- the solver behind the rational
+# functions of D^dag D in the DD-RHMC one-flavour action (eqs. 20-21)
+# ---------------------------------------------------------------------------
+def multishift_cg(orc: Oracle, b, shifts, tol, max_iter):
+    """Solves (A + sigma_i) x_i = b for all shifts with ONE Krylov space (Jegerlehner, hep-lat/9612014), written out
+    in the CG form of C8.  The base system is the smallest shift sigma_0 (slowest to converge), delta_i = sigma_i - sigma_0;
+    the residual of system i is zeta_i r, so only r is stored:
+        q = (A + sigma_0) p_0; d = <p_0, q>; alpha = c/d
+        zeta_i' = zeta_i zeta_i^old alpha^old / (alpha beta^old (zeta_i^old - zeta_i) + zeta_i^old alpha^old (1 + delta_i alpha))
+        x_i += alpha (zeta_i'/zeta_i) p_i ;  r -= alpha q ; c' = |r|^2 ; beta = c'/c
+        p_i = zeta_i' r + beta (zeta_i'/zeta_i)^2 p_i
+    stops when |r| <= tol |b| for the base system.  Returns ([x_i], info) with the true residual of every system."""
+    b = np.ascontiguousarray(b, dtype=np.complex128)
+    shifts = [float(s) for s in shifts]
+    assert all(shifts[i] <= shifts[i + 1] for i in range(len(shifts) - 1)), "shifts ascending"
+    n = len(shifts)
+    s0 = shifts[0]
+    delta = [s - s0 for s in shifts]
+    bn2 = orc.norm2(b)
+    x = [np.zeros_like(b) for _ in shifts]
+    if bn2 == 0.0:
+        return x, dict(iters=0, resid_true=[0.0] * n, converged=True)
+    r = b.copy()
+    p = [b.copy() for _ in shifts]
+    zeta, zeta_old = [1.0] * n, [1.0] * n
+    alpha_old, beta_old = 1.0, 0.0
+    c = bn2
+    target = tol * tol * bn2
+    iters = 0
+    while c > target and iters < max_iter:
+        q = orc.mdagm(p[0]) + s0 * p[0]
+        d = float(np.real(np.vdot(p[0], q)))
+        alpha = c / d
+        znew = [0.0] * n
+        for i in range(n):
+            znew[i] = zeta[i] * zeta_old[i] * alpha_old / (
+                alpha * beta_old * (zeta_old[i] - zeta[i]) + zeta_old[i] * alpha_old * (1.0 + delta[i] * alpha))
+            x[i] += (alpha * znew[i] / zeta[i]) * p[i]
+        r -= alpha * q
+        cn = orc.norm2(r)
+        beta = cn / c
+        for i in range(n):
+            p[i] = znew[i] * r + (beta * (znew[i] / zeta[i]) ** 2) * p[i]
+        zeta_old, zeta, alpha_old, beta_old, c = zeta, znew, alpha, beta, cn
+        iters += 1
+    res = [float(np.sqrt(orc.norm2(b - orc.mdagm(x[i]) - shifts[i] * x[i]) / bn2)) for i in range(n)]
+    return x, dict(iters=iters, resid_iter=float(np.sqrt(c / bn2)), resid_true=res, converged=bool(c <= target))
+
+
+# ---------------------------------------------------------------------------
 # C9: fp32 inner / fp64 outer defect correction
 # ---------------------------------------------------------------------------
 def cg_mixed(orc64: Oracle, orc32: Oracle, b, tol, max_iter, inner_tol=1e-4, max_restarts=20, x0=None):

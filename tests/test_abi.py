@@ -65,3 +65,30 @@ def test_cuda_required_and_loud(libpath):
         pytest.skip("GPU box: covered by the gpu tests")
     with pytest.raises(RuntimeError):
         api.Dwf((4, 4, 4, 4), 4, 1.8, 0.1, 1.0, 0.0)
+
+
+def test_create_rejects_bad_arguments_without_touching_cuda(libpath):
+    """Error behaviour stated in include/dwf.h: integer status, never abort; argument validation precedes every CUDA call,
+    so these run on the CPU-only box."""
+    from paper_2203_17119_b200 import api
+    lib = api.load_library()
+
+    def create(dims, Ls, cut=(0, 0, 0, 0), M5=1.8, b5=1.5):
+        h = ctypes.c_void_p()
+        st = lib.dwf_create(ctypes.byref(h), (ctypes.c_int * 4)(*dims), Ls, M5, 0.01, b5, 0.5, (ctypes.c_int * 4)(*cut))
+        assert st != api.OK and not h.value
+        return st
+
+    assert create((4, 4, 4, 5), 8) == api.EINVAL            # odd extent
+    assert create((4, 4, 4, 0), 8) == api.EINVAL
+    assert create((4, 4, 4, 4), 0) == api.EINVAL            # Ls < 1
+    assert create((4, 4, 4, 4), 33) == api.EINVAL           # Ls beyond the table size
+    assert create((4, 4, 4, 8), 8, cut=(0, 0, 0, 3)) == api.EINVAL    # cut does not divide Lt
+    assert create((4, 4, 4, 8), 8, cut=(0, 0, 0, -4)) == api.EINVAL
+    assert create((4, 4, 4, 4), 8, M5=5.0, b5=1.0) == api.EINVAL      # bee = 1 + b5 (4 - M5) = 0: Mee singular
+    assert create((256, 256, 256, 256), 16) == api.EINVAL             # beyond the 32-bit vector index range
+    assert lib.dwf_create(None, None, 8, 1.8, 0.01, 1.5, 0.5, None) == api.EINVAL
+    assert lib.dwf_destroy(None) == api.EINVAL
+    assert lib.dwf_launch_count(None) == 0
+    lib.dwf_last_error.restype = ctypes.c_char_p
+    assert lib.dwf_last_error(None) == b"null context"

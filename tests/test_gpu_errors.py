@@ -1,0 +1,60 @@
+"""Error behaviour of the C ABI on the GPU box (include/dwf.h: status codes, no abort, message in dwf_last_error)."""
+import ctypes
+
+import numpy as np
+import pytest
+
+from paper_2203_17119_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    import torch
+    assert torch.cuda.is_available()
+    from paper_2203_17119_b200 import api
+    g = api.Dwf((4, 4, 4, 8), 8, 1.8, 0.01, 1.5, 0.5)
+    yield api, g
+    g.close()
+
+
+def test_operators_need_a_gauge_field(ctx):
+    api, g = ctx
+    a, b = g.new_native(api.F64, api.ODD), g.new_native(api.F64, api.EVEN)
+    with pytest.raises(api.DwfError) as e:
+        g.dhop(a, api.EVEN, False, api.F64, out=b)
+    assert e.value.status == api.ESTATE and "gauge" in str(e.value)
+    with pytest.raises(api.DwfError) as e:
+        g.cg(a, 1e-8, 10)
+    assert e.value.status == api.ESTATE
+
+
+def test_aliasing_bad_tolerance_and_late_options(ctx):
+    api, g = ctx
+    g.set_gauge(inputs.gauge_weak((4, 4, 4, 8), 0.3, 5))
+    a = g.new_native(api.F64, api.ODD).normal_()
+    for call in (lambda: g.mpc(a, False, api.F64, out=a), lambda: g.mdagm(a, api.F64, out=a),
+                 lambda: g.mooee_inv(a, api.ODD, False, api.F64, out=a)):
+        with pytest.raises(api.DwfError) as e:
+            call()
+        assert e.value.status == api.EINVAL
+    info = api.CgInfo()
+    st = g.lib.dwf_cg(g._h, g._p(g.new_native()), g._p(a), -1.0, 10, api.CG_F64, 0, ctypes.byref(info))
+    assert st == api.EINVAL
+    with pytest.raises(api.DwfError) as e:
+        g.set_option("compress12", 0)                  # layout options are frozen once the gauge field is in
+    assert e.value.status == api.ESTATE
+    with pytest.raises(api.DwfError) as e:
+        g.set_option("no_such_option", 1)
+    assert e.value.status == api.EINVAL
+
+
+def test_max_iter_reached_is_reported_not_raised(ctx):
+    api, g = ctx
+    b = g.pack(inputs.source_half((4, 4, 4, 8), 8, 9, parity=1), api.F64, api.ODD)
+    x, info, st = g.cg(b, 1e-12, 3, api.CG_F64)
+    assert st == api.ENOTCONV and info["iters_total"] == 3 and info["resid_true"] > 1e-12
+    assert np.isfinite(g.unpack(x, api.F64, api.ODD)).all()        # x holds the best iterate
+    x, info, st = g.cg(g.new_native().zero_(), 1e-10, 100, api.CG_F64)      # b = 0: x = 0, converged at once
+    assert st == api.OK and info["iters_total"] == 0 and float(x.abs().max()) == 0.0

@@ -318,6 +318,29 @@ def test_cg_vs_dense_solve(U, psi, oracle_built):
     assert info2["iters"] == 0 and info2["converged"]
 
 
+def test_multishift_cg_vs_dense_solves(U, psi, oracle_built):
+    """NEXT-2: every shifted solution against numpy's dense solve of (Mpc^dag Mpc + sigma) x = b, the matrix built
+    from dense blocks (independent of the oracle's loops); one shared iteration count; sigma = 0 reproduces plain CG."""
+    from oracle.dwf_oracle import multishift_cg
+    par = MOEB
+    o = make(par, U)
+    M = dr.dwf_matrix(U, DIMS, LS, par["M5"], par["mf"], par["b5"], par["c5"])
+    ev, od = dr.parity_index(DIMS, LS)
+    Mpc = M[np.ix_(od, od)] - M[np.ix_(od, ev)] @ np.linalg.solve(M[np.ix_(ev, ev)], M[np.ix_(ev, od)])
+    A = Mpc.conj().T @ Mpc
+    _, b = split(psi, DIMS)
+    shifts = [0.0, 0.01, 0.3, 5.0]
+    xs, info = multishift_cg(o, b, shifts, 1e-11, 2000)
+    assert info["converged"] and max(info["resid_true"]) <= 1.01e-11
+    for x, sg in zip(xs, shifts):
+        want = np.linalg.solve(A + sg * np.eye(A.shape[0]), b.reshape(-1))
+        assert rel(x.reshape(-1), want) < 1e-9
+    # the larger the shift the better conditioned the system: true residuals do not increase with sigma
+    assert all(info["resid_true"][i + 1] <= info["resid_true"][i] * (1 + 1e-6) + 1e-15 for i in range(3))
+    x0, info0 = cg(o, b, 1e-11, 2000)
+    assert abs(info["iters"] - info0["iters"]) <= 1 and rel(xs[0], x0) < 1e-9
+
+
 def test_redblack_solve_vs_dense(U, psi, oracle_built):
     par = SHAM
     o = make(par, U)
