@@ -129,6 +129,14 @@ dwf_status dwf_norm2(dwf_ctx* ctx, const void* v_dev, dwf_prec prec, dwf_parity 
  * until |b - A x| <= tol |b|.  Returns DWF_ENOTCONV if max_iter is reached. */
 dwf_status dwf_cg(dwf_ctx* ctx, void* x_dev, const void* b_dev, double tol, int max_iter, dwf_cg_mode mode,
                   int use_guess, dwf_cg_info* info);
+/* Multishift CG (the solver behind rational functions of D^dag D in the DD-RHMC one-flavour action,
+ * eqs. 20-21): (Mpc^dag Mpc + shifts[i]) x_i = b for i < nshift with one shared Krylov space, fp64.
+ * x_dev: OUT, nshift fp64 native ODD fields back to back (field i at byte offset i * dwf_field_bytes(F64, ODD)), start
+ * from zero; b_dev: fp64 native ODD field; shifts_host: nshift <= 16 values, ascending, shifts[0] >= 0 is the base system
+ * whose recurrence residual is driven to tol |b|; resid_true_host (may be NULL): |b - (A + shift_i) x_i| / |b| recomputed
+ * at exit for every i; info->resid_true is their maximum.  Status as dwf_cg (DWF_ENOTCONV at max_iter). */
+dwf_status dwf_multishift_cg(dwf_ctx* ctx, void* x_dev, const void* b_dev, const double* shifts_host, int nshift, double tol,
+                             int max_iter, dwf_cg_info* info, double* resid_true_host);
 /* M psi = eta on FULL fp64 native fields through the red-black wrap (reading C6):
  * eta' = eta_o - Moe Mee^-1 eta_e; Mpc^dag Mpc psi_o = Mpc^dag eta'; psi_e = Mee^-1 (eta_e - Meo psi_o). */
 dwf_status dwf_solve(dwf_ctx* ctx, void* psi_dev, const void* eta_dev, double tol, int max_iter, dwf_cg_mode mode,

@@ -367,6 +367,7 @@ dwf_status dwf_destroy(dwf_ctx* c) {
     for (cudaEvent_t e : c->ev) cudaEventDestroy(e);
     pipe_tables_free(c);
     tma_state_free(c);
+    if (c->ms_p) cudaFree(c->ms_p);
     if (c->partials) cudaFree(c->partials);
     if (c->scalars) cudaFree(c->scalars);
     if (c->scalars_host) cudaFreeHost(c->scalars_host);
@@ -564,6 +565,99 @@ dwf_status dwf_cg(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, 
     info->launches = (int)(c->launches - l0);
     if (st == DWF_ENOTCONV) c->err = "cg: max_iter reached";
     return st;
+}
+
+dwf_status dwf_multishift_cg(dwf_ctx* c, void* xv, const void* b, const double* shifts, int nshift, double tol, int max_iter,
+                             dwf_cg_info* info, double* resid_true) {
+    DWF_TRY(need_gauge(c));
+    dwf_cg_info local;
+    if (!info) info = &local;
+    memset(info, 0, sizeof(*info));
+    if (!xv || !b || xv == b || !shifts || nshift < 1 || nshift > 16 || tol <= 0.0 || max_iter < 0 || shifts[0] < 0.0) {
+        c->err = "multishift_cg: bad arguments";
+        return DWF_EINVAL;
+    }
+    for (int i = 1; i < nshift; ++i)
+        if (shifts[i] < shifts[i - 1]) { c->err = "multishift_cg: shifts must ascend"; return DWF_EINVAL; }
+    const long long l0 = c->launches;
+    const double t0 = now_s();
+    const int P = DWF_F64;
+    const size_t hb = half_bytes(c->g, P), n = half_reals(c);
+    if (c->ms_p_bytes < hb * nshift) {
+        if (c->ms_p) cudaFree(c->ms_p);
+        c->ms_p = nullptr; c->ms_p_bytes = 0;
+        if (cudaMalloc(&c->ms_p, hb * nshift) != cudaSuccess) { cudaGetLastError(); c->err = "cudaMalloc(multishift) failed"; return DWF_ENOMEM; }
+        c->ms_p_bytes = hb * nshift;
+    }
+    char* x = (char*)xv;
+    char* p = (char*)c->ms_p;
+    void *r, *q, *z;
+    DWF_TRY(ws_get(c, P, 2, &r));
+    DWF_TRY(ws_get(c, P, 4, &q));
+    DWF_TRY(ws_get(c, P, 5, &z));
+    double bn2;
+    DWF_TRY(norm2_host(c, b, P, &bn2));
+    DWF_CUDA_CHECK(c, cudaMemsetAsync(x, 0, hb * nshift, c->stream));
+    if (bn2 == 0.0) {
+        if (resid_true) for (int i = 0; i < nshift; ++i) resid_true[i] = 0.0;
+        return DWF_OK;
+    }
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(r, b, hb, cudaMemcpyDeviceToDevice, c->stream));
+    for (int i = 0; i < nshift; ++i) DWF_CUDA_CHECK(c, cudaMemcpyAsync(p + i * hb, b, hb, cudaMemcpyDeviceToDevice, c->stream));
+    const double s0 = shifts[0], target = tol * tol * bn2;
+    double zeta[16], zeta_old[16], znew[16], ax[16], zr[16], bp[16];
+    for (int i = 0; i < nshift; ++i) zeta[i] = zeta_old[i] = 1.0;
+    double alpha_old = 1.0, beta_old = 0.0, cc = bn2, p0n2 = bn2;
+    int iters = 0;
+    while (cc > target && iters < max_iter) {
+        // q = Mpc p_0 (|q|^2 -> SLOT_D), z = Mpc^dag q;  d = <p_0, (A + s0) p_0> = |q|^2 + s0 |p_0|^2
+        DWF_TRY(mpc_apply(c, q, p, 0, P, SLOT_D));
+        DWF_TRY(mpc_apply(c, z, q, 1, P, -1));
+        double qn2;
+        DWF_TRY(read_slot(c, SLOT_D, &qn2));
+        const double d = qn2 + s0 * p0n2;
+        const double alpha = cc / d;
+        for (int i = 0; i < nshift; ++i) {
+            const double dl = shifts[i] - s0;
+            znew[i] = zeta[i] * zeta_old[i] * alpha_old /
+                      (alpha * beta_old * (zeta_old[i] - zeta[i]) + zeta_old[i] * alpha_old * (1.0 + dl * alpha));
+            ax[i] = alpha * znew[i] / zeta[i];
+        }
+        DWF_TRY(launch_ms_r(c, r, z, p, alpha, alpha * s0, n, SLOT_CN));        // r -= alpha (z + s0 p_0), |r|^2
+        double cn;
+        DWF_TRY(read_slot(c, SLOT_CN, &cn));
+        if (!(cn == cn)) { c->err = "multishift_cg: NaN residual"; return DWF_ECUDA; }
+        const double beta = cn / cc;
+        for (int i = 0; i < nshift; ++i) {
+            zr[i] = znew[i];
+            bp[i] = beta * (znew[i] / zeta[i]) * (znew[i] / zeta[i]);
+        }
+        DWF_TRY(launch_ms_update(c, x, p, r, n, nshift, ax, zr, bp, SLOT_T1));   // x_i += .. p_i ; p_i = .. ; |p_0|^2
+        DWF_TRY(read_slot(c, SLOT_T1, &p0n2));
+        for (int i = 0; i < nshift; ++i) { zeta_old[i] = zeta[i]; zeta[i] = znew[i]; }
+        alpha_old = alpha; beta_old = beta; cc = cn;
+        ++iters;
+    }
+    info->iters_total = iters;
+    info->resid_iter = std::sqrt(cc / bn2);
+    // true residuals: b - (A + s_i) x_i
+    double worst = 0.0;
+    for (int i = 0; i < nshift; ++i) {
+        DWF_TRY(mdagm_apply(c, z, x + i * hb, P));
+        DWF_TRY(launch_sub(c, q, b, z, P, n));
+        DWF_TRY(launch_axpy(c, q, x + i * hb, -shifts[i], P, n));
+        double rn2;
+        DWF_TRY(norm2_host(c, q, P, &rn2));
+        const double rt = std::sqrt(rn2 / bn2);
+        if (resid_true) resid_true[i] = rt;
+        if (rt > worst) worst = rt;
+    }
+    info->resid_true = worst;
+    cudaStreamSynchronize(c->stream);
+    info->seconds = now_s() - t0;
+    info->launches = (int)(c->launches - l0);
+    if (cc > target) { c->err = "multishift_cg: max_iter reached"; return DWF_ENOTCONV; }
+    return DWF_OK;
 }
 
 dwf_status dwf_solve(dwf_ctx* c, void* psi, const void* eta, double tol, int max_iter, dwf_cg_mode mode, dwf_cg_info* info) {

@@ -95,6 +95,51 @@ __global__ void __launch_bounds__(256) sub_kernel(typename VB<R>::V* __restrict_
         out[i] = axpyv((R)-1, b[i], a[i]);
 }
 
+// ---- multishift CG (dwf_multishift_cg): the residual step of the base system and one pass over all shifted systems
+// r -= a z + as0 p0 ; |r|^2
+template <typename R>
+__global__ void __launch_bounds__(256) ms_r_kernel(typename VB<R>::V* __restrict__ r, const typename VB<R>::V* __restrict__ z,
+                                                   const typename VB<R>::V* __restrict__ p0, R a, R as0, size_t nvec,
+                                                   double* __restrict__ partials) {
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        typename VB<R>::V v = axpyv(-a, z[i], r[i]);
+        v = axpyv(-as0, p0[i], v);
+        r[i] = v;
+        acc += n2(v);
+    }
+    acc = blk_sum(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x] = acc;
+}
+
+struct MsCoef {
+    int n;
+    double ax[16];    // x_i += ax_i p_i   (old p_i)
+    double zr[16];    // p_i  = zr_i r + bp_i p_i
+    double bp[16];
+};
+
+// for every shift i: x_i += ax_i p_i ; p_i = zr_i r + bp_i p_i ; |p_0|^2 of the new p_0.  r is read once.
+template <typename R>
+__global__ void __launch_bounds__(256) ms_update_kernel(typename VB<R>::V* __restrict__ x, typename VB<R>::V* __restrict__ p,
+                                                        const typename VB<R>::V* __restrict__ r, size_t nvec, MsCoef c,
+                                                        double* __restrict__ partials) {
+    double acc = 0.0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        const typename VB<R>::V rv = r[i];
+        for (int k = 0; k < c.n; ++k) {
+            const typename VB<R>::V pv = p[(size_t)k * nvec + i];
+            x[(size_t)k * nvec + i] = axpyv((R)c.ax[k], pv, x[(size_t)k * nvec + i]);
+            typename VB<R>::V pn = axpyv((R)c.bp[k], pv, typename VB<R>::V{});
+            pn = axpyv((R)c.zr[k], rv, pn);
+            p[(size_t)k * nvec + i] = pn;
+            if (k == 0) acc += n2(pn);
+        }
+    }
+    acc = blk_sum(acc);
+    if (threadIdx.x == 0) partials[blockIdx.x] = acc;
+}
+
 static inline int blas_grid(size_t nvec) {
     size_t want = (nvec + 255) / 256;
     size_t cap = 148 * 8;                    // 8 CTAs of 256 threads per SM, one wave
@@ -166,6 +211,34 @@ dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int p
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
     return DWF_OK;
+}
+
+// r -= a z + a s0 p0, |r|^2 -> scalars[slot]   (fp64 fields)
+dwf_status launch_ms_r(dwf_ctx* c, void* r, const void* z, const void* p0, double a, double as0, size_t nreal, int slot) {
+    const size_t nvec = nreal / 2;
+    const int grid = blas_grid(nvec);
+    dwf_status st = ensure_partials(c, grid);
+    if (st != DWF_OK) return st;
+    ms_r_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)r, (const double2*)z, (const double2*)p0, a, as0, nvec, c->partials);
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return launch_reduce(c, grid, slot);
+}
+
+// all shifts at once (fields i at x + i*nreal, p + i*nreal); |p_0|^2 -> scalars[slot]
+dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t nreal, int n, const double* ax, const double* zr,
+                            const double* bp, int slot) {
+    const size_t nvec = nreal / 2;
+    const int grid = blas_grid(nvec);
+    dwf_status st = ensure_partials(c, grid);
+    if (st != DWF_OK) return st;
+    MsCoef co;
+    co.n = n;
+    for (int i = 0; i < 16; ++i) { co.ax[i] = i < n ? ax[i] : 0.0; co.zr[i] = i < n ? zr[i] : 0.0; co.bp[i] = i < n ? bp[i] : 0.0; }
+    ms_update_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)x, (double2*)p, (const double2*)r, nvec, co, c->partials);
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return launch_reduce(c, grid, slot);
 }
 
 }  // namespace dwf

@@ -84,6 +84,8 @@ struct dwf_ctx {
     // workspace (allocated lazily, sized for half fields)
     void* ws64[10] = {};
     void* ws32[10] = {};
+    void* ms_p = nullptr;        // multishift CG: search directions of all shifts
+    size_t ms_p_bytes = 0;
     double* partials = nullptr;  // per-block reduction partials
     int npartials = 0;
     double* scalars = nullptr;   // device scalars
@@ -131,6 +133,9 @@ dwf_status launch_xpay(dwf_ctx* c, void* p, const void* r, int prec, size_t nrea
 dwf_status launch_axpy(dwf_ctx* c, void* y, const void* x, double a, int prec, size_t nreal);  // y += a x
 dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int prec, size_t nreal);  // out = a - b
 dwf_status launch_add_f32_to_f64(dwf_ctx* c, void* x64, const void* e32, size_t unused);  // x += (double)e, half field
+dwf_status launch_ms_r(dwf_ctx* c, void* r, const void* z, const void* p0, double a, double as0, size_t nreal, int slot);
+dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t nreal, int n, const double* ax, const double* zr,
+                            const double* bp, int slot);
 dwf_status ensure_partials(dwf_ctx* c, int n);
 dwf_status launch_reduce(dwf_ctx* c, int n, int slot);
 void build_tables(dwf_ctx* c);

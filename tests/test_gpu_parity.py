@@ -239,3 +239,26 @@ def test_host_entry_points(case):
     _, info, st = g.solve_host(psi, src, 1e-9, 5000, A.CG_F64)
     assert st == A.OK
     assert np.sqrt(case.orc.norm2(case.full - case.orc.M(psi)) / case.orc.norm2(case.full)) < 1e-6
+
+
+def test_multishift_cg_matches_oracle(case):
+    """NEXT-2 (eqs. 20-21): all shifted solutions of (Mpc^dag Mpc + sigma_i) x_i = b against the
+    oracle's multishift CG, shared iteration count within +-2, true residuals recomputed by the oracle."""
+    from oracle.dwf_oracle import multishift_cg
+    g, A = case.gpu, case.api
+    if int(np.prod(case.dims)) * case.Ls > 30000:
+        pytest.skip("the oracle's multishift CG takes minutes on this lattice; the smaller ones cover every code path")
+    shifts = [0.0, 0.02, 0.4, 3.0]
+    tol = 1e-10
+    xs_ref, info_ref = multishift_cg(case.orc, case.odd, shifts, tol, 5000)
+    xs, info, res, st = g.multishift_cg(g.pack(case.odd, A.F64, A.ODD), shifts, tol, 5000)
+    assert st == A.OK and info_ref["converged"]
+    assert abs(info["iters_total"] - info_ref["iters"]) <= 2, (info, info_ref)
+    bn2 = case.orc.norm2(case.odd)
+    for x, xr, sg, rt in zip(xs, xs_ref, shifts, res):
+        got = g.unpack(x, A.F64, A.ODD)
+        assert rel(got, xr) < 1e-6
+        true_res = np.sqrt(case.orc.norm2(case.odd - case.orc.mdagm(got) - sg * got) / bn2)
+        assert true_res <= 2 * tol and abs(true_res - rt) <= 1e-3 * true_res + 1e-14
+    with pytest.raises(A.DwfError):
+        g.multishift_cg(g.pack(case.odd, A.F64, A.ODD), [0.5, 0.1], tol, 10)       # shifts must ascend
