@@ -267,6 +267,25 @@ def multishift_cg(orc: Oracle, b, shifts, tol, max_iter):
 
 
 # ---------------------------------------------------------------------------
+# NEXT-4: Chebyshev polynomial of A = Mpc^dag Mpc applied to a vector -- the "filter functions ... which
+# can be obtained recursively" of the paper's multigrid set-up (Fig. 4 caption PAPER.md:191).  The paper
+# gives neither window nor order: both are arguments.
+# ---------------------------------------------------------------------------
+def chebyshev(orc: Oracle, v, lo, hi, order):
+    """T_n(a) v with a = (2A - (hi + lo)) / (hi - lo), by the three-term recurrence
+    t_0 = v, t_1 = a v, t_{k+1} = 2 a t_k - t_{k-1}."""
+    v = np.ascontiguousarray(v, dtype=np.complex128)
+    s, o = 2.0 / (hi - lo), -(hi + lo) / (hi - lo)
+    amul = lambda x: s * orc.mdagm(x) + o * x
+    if order == 0:
+        return v.copy()
+    t0, t1 = v, amul(v)
+    for _ in range(order - 1):
+        t0, t1 = t1, 2.0 * amul(t1) - t0
+    return t1
+
+
+# ---------------------------------------------------------------------------
 # C9: fp32 inner / fp64 outer defect correction
 # ---------------------------------------------------------------------------
 def cg_mixed(orc64: Oracle, orc32: Oracle, b, tol, max_iter, inner_tol=1e-4, max_restarts=20, x0=None):

@@ -341,6 +341,31 @@ def test_multishift_cg_vs_dense_solves(U, psi, oracle_built):
     assert abs(info["iters"] - info0["iters"]) <= 1 and rel(xs[0], x0) < 1e-9
 
 
+def test_chebyshev_filter_vs_spectral_decomposition(U, psi, oracle_built):
+    """NEXT-4: T_n((2A - hi - lo)/(hi - lo)) v against the spectral definition sum_i T_n(l_i) <u_i, v> u_i from numpy's
+    eigh of the dense Mpc^dag Mpc and numpy's own Chebyshev evaluation (no recurrence shared with the oracle)."""
+    from numpy.polynomial import chebyshev as npcheb
+    from oracle.dwf_oracle import chebyshev
+    par = MOEB
+    o = make(par, U)
+    M = dr.dwf_matrix(U, DIMS, LS, par["M5"], par["mf"], par["b5"], par["c5"])
+    ev, od = dr.parity_index(DIMS, LS)
+    Mpc = M[np.ix_(od, od)] - M[np.ix_(od, ev)] @ np.linalg.solve(M[np.ix_(ev, ev)], M[np.ix_(ev, od)])
+    lam, Uv = np.linalg.eigh(Mpc.conj().T @ Mpc)
+    _, b = split(psi, DIMS)
+    lo, hi = 0.5 * lam[-1], 1.05 * lam[-1]          # a window on the upper part of the spectrum: low modes are amplified
+    for n in (0, 1, 2, 7, 16):
+        coef = np.zeros(n + 1)
+        coef[n] = 1.0
+        tl = npcheb.chebval((2 * lam - (hi + lo)) / (hi - lo), coef)
+        want = Uv @ (tl * (Uv.conj().T @ b.reshape(-1)))
+        got = chebyshev(o, b, lo, hi, n).reshape(-1)
+        assert rel(got, want) < 1e-9, n
+    # inside the window |T_n| <= 1, below it the filter grows: the lowest mode is enhanced relative to the top one
+    gain = npcheb.chebval((2 * lam[[0, -1]] - (hi + lo)) / (hi - lo), coef)
+    assert abs(gain[0]) > 1e3 * abs(gain[1])
+
+
 def test_redblack_solve_vs_dense(U, psi, oracle_built):
     par = SHAM
     o = make(par, U)
