@@ -137,6 +137,11 @@ dwf_status dwf_cg(dwf_ctx* ctx, void* x_dev, const void* b_dev, double tol, int 
  * at exit for every i; info->resid_true is their maximum.  Status as dwf_cg (DWF_ENOTCONV at max_iter). */
 dwf_status dwf_multishift_cg(dwf_ctx* ctx, void* x_dev, const void* b_dev, const double* shifts_host, int nshift, double tol,
                              int max_iter, dwf_cg_info* info, double* resid_true_host);
+/* Chebyshev polynomial filter (the recursively obtained filter functions of the paper's multigrid
+ * set-up, Fig. 4 caption PAPER.md:191 and PAPER.md:197): out = T_order(a) in with a = (2 A - (hi + lo)) / (hi - lo),
+ * A = Mpc^dag Mpc, by t_0 = in, t_1 = a in, t_{k+1} = 2 a t_k - t_{k-1}.  Native ODD fields of precision prec, device
+ * pointers, out != in; hi > lo; order >= 0.  Enqueued on the context stream (no synchronisation). */
+dwf_status dwf_chebyshev(dwf_ctx* ctx, void* out_dev, const void* in_dev, double lo, double hi, int order, dwf_prec prec);
 /* M psi = eta on FULL fp64 native fields through the red-black wrap (reading C6):
  * eta' = eta_o - Moe Mee^-1 eta_e; Mpc^dag Mpc psi_o = Mpc^dag eta'; psi_e = Mee^-1 (eta_e - Meo psi_o). */
 dwf_status dwf_solve(dwf_ctx* ctx, void* psi_dev, const void* eta_dev, double tol, int max_iter, dwf_cg_mode mode,

@@ -660,6 +660,36 @@ dwf_status dwf_multishift_cg(dwf_ctx* c, void* xv, const void* b, const double* 
     return DWF_OK;
 }
 
+dwf_status dwf_chebyshev(dwf_ctx* c, void* out, const void* in, double lo, double hi, int order, dwf_prec prec) {
+    DWF_TRY(need_gauge(c));
+    if (!out || !in || out == in || !(hi > lo) || order < 0) { c->err = "chebyshev: bad arguments"; return DWF_EINVAL; }
+    const size_t hb = half_bytes(c->g, prec), n = half_reals(c);
+    const double s = 2.0 / (hi - lo), o = -(hi + lo) / (hi - lo);
+    if (order == 0) {
+        DWF_CUDA_CHECK(c, cudaMemcpyAsync(out, in, hb, cudaMemcpyDeviceToDevice, c->stream));
+        return DWF_OK;
+    }
+    void *ta, *tb, *av;
+    DWF_TRY(ws_get(c, prec, 6, &av));
+    DWF_TRY(ws_get(c, prec, 7, &ta));
+    DWF_TRY(ws_get(c, prec, 8, &tb));
+    // t_1 = s A in + o in
+    DWF_TRY(mdagm_apply(c, av, in, prec));
+    void* t1 = (order == 1) ? out : ta;
+    DWF_TRY(launch_lincomb3(c, t1, av, in, in, s, o, 0.0, prec, n));
+    const void* tkm1 = in;          // t_{k-1}
+    void* tk = t1;                  // t_k
+    for (int k = 1; k < order; ++k) {
+        // t_{k+1} = 2 s A t_k + 2 o t_k - t_{k-1}, written over the buffer that is free (never over `in`)
+        DWF_TRY(mdagm_apply(c, av, tk, prec));
+        void* dst = (k + 1 == order) ? out : ((tk == ta) ? tb : ta);
+        DWF_TRY(launch_lincomb3(c, dst, av, tk, tkm1, 2.0 * s, 2.0 * o, -1.0, prec, n));
+        tkm1 = tk;
+        tk = dst;
+    }
+    return DWF_OK;
+}
+
 dwf_status dwf_solve(dwf_ctx* c, void* psi, const void* eta, double tol, int max_iter, dwf_cg_mode mode, dwf_cg_info* info) {
     DWF_TRY(need_gauge(c));
     dwf_cg_info local;

@@ -140,6 +140,18 @@ __global__ void __launch_bounds__(256) ms_update_kernel(typename VB<R>::V* __res
     if (threadIdx.x == 0) partials[blockIdx.x] = acc;
 }
 
+// out = a x + b y + c z   (Chebyshev recurrence step; out may alias z)
+template <typename R>
+__global__ void __launch_bounds__(256) lincomb3_kernel(typename VB<R>::V* out, const typename VB<R>::V* __restrict__ x,
+                                                       const typename VB<R>::V* __restrict__ y, const typename VB<R>::V* z, R a,
+                                                       R b, R c, size_t nvec) {
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
+        typename VB<R>::V v = axpyv(c, z[i], typename VB<R>::V{});
+        v = axpyv(b, y[i], v);
+        out[i] = axpyv(a, x[i], v);
+    }
+}
+
 static inline int blas_grid(size_t nvec) {
     size_t want = (nvec + 255) / 256;
     size_t cap = 148 * 8;                    // 8 CTAs of 256 threads per SM, one wave
@@ -239,6 +251,22 @@ dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t 
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
     return launch_reduce(c, grid, slot);
+}
+
+dwf_status launch_lincomb3(dwf_ctx* c, void* out, const void* x, const void* y, const void* z, double a, double b, double cc,
+                           int prec, size_t nreal) {
+    if (prec == DWF_F64) {
+        const size_t nvec = nreal / 2;
+        lincomb3_kernel<double><<<blas_grid(nvec), 256, 0, c->stream>>>((double2*)out, (const double2*)x, (const double2*)y,
+                                                                        (const double2*)z, a, b, cc, nvec);
+    } else {
+        const size_t nvec = nreal / 4;
+        lincomb3_kernel<float><<<blas_grid(nvec), 256, 0, c->stream>>>((float4*)out, (const float4*)x, (const float4*)y,
+                                                                       (const float4*)z, (float)a, (float)b, (float)cc, nvec);
+    }
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
 }
 
 }  // namespace dwf

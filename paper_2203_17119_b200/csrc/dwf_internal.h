@@ -136,6 +136,8 @@ dwf_status launch_add_f32_to_f64(dwf_ctx* c, void* x64, const void* e32, size_t 
 dwf_status launch_ms_r(dwf_ctx* c, void* r, const void* z, const void* p0, double a, double as0, size_t nreal, int slot);
 dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t nreal, int n, const double* ax, const double* zr,
                             const double* bp, int slot);
+dwf_status launch_lincomb3(dwf_ctx* c, void* out, const void* x, const void* y, const void* z, double a, double b, double cc,
+                           int prec, size_t nreal);   // out = a x + b y + cc z
 dwf_status ensure_partials(dwf_ctx* c, int n);
 dwf_status launch_reduce(dwf_ctx* c, int n, int slot);
 void build_tables(dwf_ctx* c);

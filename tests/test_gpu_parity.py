@@ -262,3 +262,20 @@ def test_multishift_cg_matches_oracle(case):
         assert true_res <= 2 * tol and abs(true_res - rt) <= 1e-3 * true_res + 1e-14
     with pytest.raises(A.DwfError):
         g.multishift_cg(g.pack(case.odd, A.F64, A.ODD), [0.5, 0.1], tol, 10)       # shifts must ascend
+
+
+@pytest.mark.parametrize("prec", ["f64", "f32"])
+def test_chebyshev_filter_matches_oracle(case, prec):
+    """NEXT-4 (SURVEY 8f; Fig. 4 caption PAPER.md:191, :197): T_n of the window-mapped Mpc^dag Mpc applied to a vector."""
+    from oracle.dwf_oracle import chebyshev
+    g, P, A = case.gpu, case.P(prec), case.api
+    orc = case.oracle(prec)
+    o = case.src(case.odd, prec)
+    rq = float(np.real(np.vdot(o, orc.mdagm(o))) / orc.norm2(o))       # a Rayleigh quotient sets the scale of the window
+    lo, hi = 0.0, 4.0 * rq
+    nat = g.pack(o, P, A.ODD)
+    for order in (0, 1, 2, 5):
+        got = g.unpack(g.chebyshev(nat, lo, hi, order, P), P, A.ODD)
+        assert rel(got, chebyshev(orc, o, lo, hi, order)) < (1e-11 if prec == "f64" else 2e-5), order
+    with pytest.raises(A.DwfError):
+        g.chebyshev(nat, 1.0, 1.0, 3, P)
