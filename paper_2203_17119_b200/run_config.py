@@ -34,7 +34,7 @@ def _time(fn, reps):
     return s.elapsed_time(e) / reps
 
 
-def run(cfg, U, b_np, with_sweeps=True, max_iter=50000):
+def run(cfg, U, b_np, with_sweeps=True, max_iter=50000, extras=False):
     A = api
     g = api.from_config(cfg)
     g.set_gauge(U)
@@ -56,6 +56,19 @@ def run(cfg, U, b_np, with_sweeps=True, max_iter=50000):
         rep[name] = {"tol": cfg.tol, "status": int(st), "iters": info["iters_total"], "restarts": info["restarts"],
                      "resid_true": info["resid_true"], "seconds": info["seconds"], "launches": info["launches"]}
         del x
+    if extras:
+        # SURVEY 8f NEXT-2 / NEXT-4 at full size: four shifts in one Krylov space; a 16th-order Chebyshev filter
+        shifts = [0.0, 0.01, 0.1, 1.0]
+        xs, info, res, st = g.multishift_cg(b, shifts, cfg.tol, max_iter)
+        rep["multishift_cg"] = {"shifts": shifts, "tol": cfg.tol, "status": int(st), "iters": info["iters_total"],
+                                "resid_true": res, "seconds": info["seconds"], "launches": info["launches"]}
+        del xs
+        for prec, name in ((A.F32, "f32"), (A.F64, "f64")):
+            v = g.new_native(prec, A.ODD).normal_()
+            out = g.new_native(prec, A.ODD)
+            ms = _time(lambda: g.chebyshev(v, 0.0, 60.0, 16, prec, out=out), 3)
+            rep[f"chebyshev16_{name}"] = {"ms": ms, "gflops": 16 * 2 * FLOP_MPC * n5h / ms / 1e6}
+            del v, out
     g.close()
     return rep
 
@@ -64,6 +77,7 @@ def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("config", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--no-uncut", action="store_true", help="cut configurations: skip the uncut comparison solve")
+    ap.add_argument("--extras", action="store_true", help="also time the multishift CG (4 shifts) and a 16th-order Chebyshev filter")
     args = ap.parse_args()
     if not torch.cuda.is_available():
         raise SystemExit("run_config needs a CUDA device: the hot path has no CPU fallback")
@@ -73,7 +87,7 @@ def main():
     b = inputs.source_half(cfg.dims, cfg.Ls, cfg.source_seed, parity=1)
     out = {"config": cfg.name, "params": {"M5": cfg.M5, "mf": cfg.mf, "b5": cfg.b5, "c5": cfg.c5, "gauge": cfg.gauge, "eps": cfg.eps},
            "plaquette": inputs.plaquette(U), "input_seconds": time.perf_counter() - t0}
-    out["as_configured"] = run(cfg, U, b)
+    out["as_configured"] = run(cfg, U, b, extras=args.extras)
     if any(cfg.cut) and not args.no_uncut:
         out["uncut_operator"] = run(dataclasses.replace(cfg, cut=(0, 0, 0, 0)), U, b, with_sweeps=False)
     print(json.dumps(out), flush=True)
