@@ -282,6 +282,8 @@ void choose_tiles(dwf_ctx* c) {
         g.T[mu] = t;
         g.NT[mu] = g.L[mu] / t;
     }
+    g.swz = 0;
+    c->swz64 = (g.T[0] == 4 && g.T[1] == 4 && g.T[2] == 4 && g.T[3] == 4) ? 1 : 0;
     g.TS = g.T[0] * g.T[1] * g.T[2] * g.T[3] / 2;
     g.ntiles = g.NT[0] * g.NT[1] * g.NT[2] * g.NT[3];
     g.Vh = g.ntiles * g.TS;

@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(256) dhop_kernel(Geom g, const typename VT<R>:
 template <typename R, int SC, int NG>
 static dwf_status launch_t(dwf_ctx* c, void* out, const void* in, const void* W, int out_parity, int dagger) {
     using V = typename VT<R>::V;
-    const Geom& g = c->g;
+    const Geom g = geom_prec(c, sizeof(R) == 8 ? DWF_F64 : DWF_F32);
     const int nchunks = (g.Ls + SC - 1) / SC;
     int block = 128;
     if (g.TS < block) block = ((g.TS + 31) / 32) * 32;

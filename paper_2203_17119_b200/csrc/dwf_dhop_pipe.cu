@@ -33,9 +33,7 @@ struct PipeTables {
     std::vector<uint16_t> slot_lane;  // [2][nslot]
 };
 
-static int lane_of_local(const Geom& g, const int y[4]) {
-    return ((y[3] * g.T[2] + y[2]) * g.T[1] + y[1]) * (g.T[0] >> 1) + (y[0] >> 1);
-}
+static int lane_of_local(const Geom& g, const int y[4]) { return lane_from_local(g, y); }
 
 static PipeTables build_pipe_tables(const Geom& g) {
     PipeTables t;
@@ -50,14 +48,8 @@ static PipeTables build_pipe_tables(const Geom& g) {
         std::vector<std::vector<int>> src(8);   // source lanes per face
         std::vector<int> want((size_t)8 * TS, -1);
         for (int lane = 0; lane < TS; ++lane) {
-            const int txh_n = g.T[0] >> 1;
-            int r = lane;
             int x[4];
-            const int txh = r % txh_n; r /= txh_n;
-            x[1] = r % g.T[1]; r /= g.T[1];
-            x[2] = r % g.T[2]; r /= g.T[2];
-            x[3] = r;
-            x[0] = 2 * txh + ((p + x[1] + x[2] + x[3]) & 1);
+            local_from_lane(g, lane, p, x);
             t.slot_lane[(size_t)p * t.nslot + lane] = (uint16_t)lane;
             for (int leg = 0; leg < 8; ++leg) {
                 const int mu = leg >> 1;
@@ -94,25 +86,28 @@ static PipeTables build_pipe_tables(const Geom& g) {
 // device copies live in the context (dwf_internal.h: pipe_*)
 dwf_status pipe_tables_upload(dwf_ctx* c) {
     pipe_tables_free(c);
-    const Geom& g = c->g;
     for (int mu = 0; mu < 4; ++mu)
-        if (g.T[mu] & 1) return DWF_OK;       // odd tile extents: generic kernel only
-    PipeTables t = build_pipe_tables(g);
-    c->pipe_nslot = t.nslot;
-    DWF_CUDA_CHECK(c, cudaMalloc(&c->pipe_nbslot, t.nbslot.size() * sizeof(uint16_t)));
-    DWF_CUDA_CHECK(c, cudaMalloc(&c->pipe_slot_dir, t.slot_dir.size() * sizeof(int16_t)));
-    DWF_CUDA_CHECK(c, cudaMalloc(&c->pipe_slot_lane, t.slot_lane.size() * sizeof(uint16_t)));
-    DWF_CUDA_CHECK(c, cudaMemcpy(c->pipe_nbslot, t.nbslot.data(), t.nbslot.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
-    DWF_CUDA_CHECK(c, cudaMemcpy(c->pipe_slot_dir, t.slot_dir.data(), t.slot_dir.size() * sizeof(int16_t), cudaMemcpyHostToDevice));
-    DWF_CUDA_CHECK(c, cudaMemcpy(c->pipe_slot_lane, t.slot_lane.data(), t.slot_lane.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        if (c->g.T[mu] & 1) return DWF_OK;       // odd tile extents: generic kernel only
+    for (int pr = 0; pr < 2; ++pr) {            // 0: fp32 fields, 1: fp64 fields (lane orders differ, geom_prec)
+        PipeTables t = build_pipe_tables(geom_prec(c, pr ? DWF_F64 : DWF_F32));
+        c->pipe_nslot = t.nslot;
+        DWF_CUDA_CHECK(c, cudaMalloc(&c->pipe_nbslot[pr], t.nbslot.size() * sizeof(uint16_t)));
+        DWF_CUDA_CHECK(c, cudaMalloc(&c->pipe_slot_dir[pr], t.slot_dir.size() * sizeof(int16_t)));
+        DWF_CUDA_CHECK(c, cudaMalloc(&c->pipe_slot_lane[pr], t.slot_lane.size() * sizeof(uint16_t)));
+        DWF_CUDA_CHECK(c, cudaMemcpy(c->pipe_nbslot[pr], t.nbslot.data(), t.nbslot.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        DWF_CUDA_CHECK(c, cudaMemcpy(c->pipe_slot_dir[pr], t.slot_dir.data(), t.slot_dir.size() * sizeof(int16_t), cudaMemcpyHostToDevice));
+        DWF_CUDA_CHECK(c, cudaMemcpy(c->pipe_slot_lane[pr], t.slot_lane.data(), t.slot_lane.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+    }
     return DWF_OK;
 }
 
 void pipe_tables_free(dwf_ctx* c) {
-    if (c->pipe_nbslot) cudaFree(c->pipe_nbslot);
-    if (c->pipe_slot_dir) cudaFree(c->pipe_slot_dir);
-    if (c->pipe_slot_lane) cudaFree(c->pipe_slot_lane);
-    c->pipe_nbslot = nullptr; c->pipe_slot_dir = nullptr; c->pipe_slot_lane = nullptr;
+    for (int pr = 0; pr < 2; ++pr) {
+        if (c->pipe_nbslot[pr]) cudaFree(c->pipe_nbslot[pr]);
+        if (c->pipe_slot_dir[pr]) cudaFree(c->pipe_slot_dir[pr]);
+        if (c->pipe_slot_lane[pr]) cudaFree(c->pipe_slot_lane[pr]);
+        c->pipe_nbslot[pr] = nullptr; c->pipe_slot_dir[pr] = nullptr; c->pipe_slot_lane[pr] = nullptr;
+    }
     c->pipe_nslot = 0;
 }
 
@@ -349,14 +344,15 @@ static dwf_status launch_pipe_ng(dwf_ctx* c, const PipeArgs& a) {
 // returns DWF_OK and sets *handled = true when a pipelined instantiation exists for this tile shape
 dwf_status launch_dhop_pipe(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec, bool* handled) {
     *handled = false;
-    if (!c->pipe_nbslot || c->g.Ls < 1) return DWF_OK;
-    const Geom& g = c->g;
+    const int pr = (prec == DWF_F64) ? 1 : 0;
+    if (!c->pipe_nbslot[pr] || c->g.Ls < 1) return DWF_OK;
+    const Geom g = geom_prec(c, prec);
     PipeArgs a;
     a.g = g; a.in = in; a.out = out;
     a.W = (prec == DWF_F64) ? c->W64[out_parity] : c->W32[out_parity];
-    a.nbslot = c->pipe_nbslot + (size_t)out_parity * 8 * g.TS;
-    a.slot_dir = c->pipe_slot_dir + (size_t)out_parity * c->pipe_nslot;
-    a.slot_lane = c->pipe_slot_lane + (size_t)out_parity * c->pipe_nslot;
+    a.nbslot = c->pipe_nbslot[pr] + (size_t)out_parity * 8 * g.TS;
+    a.slot_dir = c->pipe_slot_dir[pr] + (size_t)out_parity * c->pipe_nslot;
+    a.slot_lane = c->pipe_slot_lane[pr] + (size_t)out_parity * c->pipe_nslot;
     a.out_parity = out_parity; a.dagger = dagger;
     const int TS = g.TS, NS = c->pipe_nslot;
     const int nst = c->dhop_nst;

@@ -40,12 +40,15 @@ constexpr int NREG = 12;      // regions per stage
 
 struct TmaTables {
     std::vector<uint16_t> off;     // [2][8][128]  stage offset (16-byte units, k = 0) of the leg's neighbour
-    std::vector<uint8_t> xsrc;     // [2][2][32]   source lane (in the +x / -x tile) of each x-face slot
+    std::vector<uint8_t> gsrc;     // [2][4][32]   gathered faces (+x, -x, +y, -y): source lane in the neighbour tile
+    std::vector<uint16_t> gdst;    // [2][4][32]   ... and its stage offset (16-byte units, k = 0)
+    std::vector<uint8_t> xsrc;     // [2][2][32]   plain order (fp32): source lane (in the +x / -x tile) of each x-face slot
 };
 
-inline int lane_of(int tx, int ty, int tz, int tt) { return ((tt * 4 + tz) * 4 + ty) * 2 + (tx >> 1); }
+inline int lane_of_plain(int tx, int ty, int tz, int tt) { return ((tt * 4 + tz) * 4 + ty) * 2 + (tx >> 1); }
 
-TmaTables build_tma_tables(int K) {
+// fp32 fields: plain lane order, +-y faces by TMA boxes, +-x faces gathered (the kernel has no registers for more)
+TmaTables build_tma_tables_plain(int K) {
     TmaTables t;
     t.off.assign(2 * 8 * TSV, 0);
     t.xsrc.assign(2 * 2 * 32, 0);
@@ -60,7 +63,7 @@ TmaTables build_tma_tables(int K) {
                     else                               t.xsrc[(p * 2 + 1) * 32 + (row >> 1)] = (uint8_t)(row * 2 + 1);   // -x tile, tx = 3
                     for (int txh = 0; txh < 2; ++txh) {
                         const int tx = 2 * txh + ((p + ty + tz + tt) & 1);
-                        const int lane = lane_of(tx, ty, tz, tt);
+                        const int lane = lane_of_plain(tx, ty, tz, tt);
                         for (int leg = 0; leg < 8; ++leg) {
                             const int mu = leg >> 1;
                             int y[4] = {tx, ty, tz, tt};
@@ -82,6 +85,83 @@ TmaTables build_tma_tables(int K) {
                         }
                     }
                 }
+    }
+    return t;
+}
+
+
+// lane order of dwf_layout.cuh for 4^4 tiles: y rows XOR-rotated by tz
+inline int lane_of(int tx, int ty, int tz, int tt) { return ((tt * 4 + tz) * 4 + (ty ^ tz)) * 2 + (tx >> 1); }
+
+// Shared-memory slots.  A region is [K][32 slots] of 16-byte vectors, so slot mod 8 is the bank group of a 128-bit
+// access.  With the XOR-rotated lane order the 8 lanes of a quarter warp (one (tz, tt), all ty, both tx halves) read,
+// for every leg, 6 or 8 interior / TMA-written slots in distinct bank groups, and the face lanes miss exactly the
+// groups 2 (ty ^ tz) + {0, 1} (y legs) or 2 (ty ^ tz) + (0: +x, 1: -x) (x legs).  The x and y faces are written by
+// cp.async gathers, free to put every face site into a slot of exactly that group: the +-y faces in their own regions
+// (4 sites per group), the +-x faces interleaved over regions 10 and 11 (+x the even groups, -x the odd ones, 8 sites
+// per group).  Result: no shared-memory bank conflict on any leg (it was 1.44 wavefronts per ideal one).
+// fp64 fields: XOR-rotated lane order, conflict-free slots (see above)
+TmaTables build_tma_tables_swz(int K) {
+    TmaTables t;
+    t.off.assign(2 * 8 * TSV, 0);
+    t.gsrc.assign(2 * 4 * 32, 0);
+    t.gdst.assign(2 * 4 * 32, 0);
+    for (int p = 0; p < 2; ++p) {
+        const int q = 1 - p;   // input parity
+        // ---- slots of the gathered faces: face f = 0 (+x: sites tx = 0 of the +x tile), 1 (-x: tx = 3), 2 (+y: ty = 0), 3 (-y: ty = 3)
+        int slot_of[4][4][4][4];          // [f][tt][tz][u]: u = ty for x faces, tx/2 for y faces; -1 = not a site of parity q
+        int cnt[4][8];
+        memset(cnt, 0, sizeof(cnt));
+        int nface[4] = {0, 0, 0, 0};
+        for (int f = 0; f < 4; ++f)
+            for (int tt = 0; tt < 4; ++tt)
+                for (int tz = 0; tz < 4; ++tz)
+                    for (int u = 0; u < 4; ++u) {
+                        slot_of[f][tt][tz][u] = -1;
+                        int tx, ty;
+                        if (f < 2) { tx = (f == 0) ? 0 : 3; ty = u; if (((q + tx + ty + tz + tt) & 1) != 0) continue; }
+                        else { if (u >= 2) continue; ty = (f == 2) ? 0 : 3; tx = 2 * u + ((q + ty + tz + tt) & 1); }
+                        const int pos = ty ^ tz;
+                        int region, slot;
+                        if (f < 2) {
+                            const int b = 2 * pos + f;                       // +x even groups, -x odd groups
+                            const int s64 = b + 8 * cnt[f][b]++;
+                            region = 10 + (s64 >> 5); slot = s64 & 31;
+                        } else {
+                            const int b = 2 * pos + (tx >> 1);
+                            slot = b + 8 * cnt[f][b]++;
+                            region = (f == 2) ? 8 : 9;
+                        }
+                        slot_of[f][tt][tz][u] = region * K * 32 + slot;
+                        const int i = nface[f]++;
+                        t.gsrc[(p * 4 + f) * 32 + i] = (uint8_t)lane_of(tx, ty, tz, tt);
+                        t.gdst[(p * 4 + f) * 32 + i] = (uint16_t)(region * K * 32 + slot);
+                    }
+        // ---- every output site's 8 neighbours
+        for (int tt = 0; tt < 4; ++tt)
+            for (int tz = 0; tz < 4; ++tz)
+                for (int ty = 0; ty < 4; ++ty)
+                    for (int txh = 0; txh < 2; ++txh) {
+                        const int tx = 2 * txh + ((p + ty + tz + tt) & 1);
+                        const int lane = lane_of(tx, ty, tz, tt);
+                        for (int leg = 0; leg < 8; ++leg) {
+                            const int mu = leg >> 1;
+                            int y[4] = {tx, ty, tz, tt};
+                            y[mu] += (leg & 1) ? -1 : +1;
+                            int o;
+                            if (y[mu] >= 0 && y[mu] < 4) {
+                                o = y[3] * K * 32 + (lane_of(y[0], y[1], y[2], y[3]) & 31);          // own slab y[3]
+                            } else {
+                                const int up = (y[mu] >= 4);
+                                y[mu] = (y[mu] + 4) & 3;
+                                if (mu == 3)      o = (up ? 4 : 5) * K * 32 + (lane_of(y[0], y[1], y[2], 0) & 31);   // t face: one slab
+                                else if (mu == 2) o = (up ? 6 : 7) * K * 32 + y[3] * 8 + (y[1] ^ y[2]) * 2 + (y[0] >> 1);  // z face: 8 lanes x tt
+                                else if (mu == 1) o = slot_of[up ? 2 : 3][y[3]][y[2]][y[0] >> 1];
+                                else              o = slot_of[up ? 0 : 1][y[3]][y[2]][y[1]];
+                            }
+                            t.off[(p * 8 + leg) * TSV + lane] = (uint16_t)o;
+                        }
+                    }
     }
     return t;
 }
@@ -156,7 +236,9 @@ EncodeTiledFn encode_fn() {
 
 struct TmaState {
     uint16_t* off = nullptr;      // device [2][8][128]
-    uint8_t* xsrc = nullptr;      // device [2][2][32]
+    uint8_t* xsrc = nullptr;      // device [2][2][32]   (fp32 path)
+    uint8_t* gsrc = nullptr;      // device [2][4][32]   (fp64 path)
+    uint16_t* gdst = nullptr;     // device [2][4][32]   (fp64 path)
     uint32_t* order = nullptr;    // device [ntiles]
     int* counters = nullptr;      // device [3]: next position in `order`, CTAs done, round arrivals (self-resetting, see the kernel)
     int K_built = 0;
@@ -170,6 +252,8 @@ void tma_state_free(dwf_ctx* c) {
     if (!s) return;
     if (s->off) cudaFree(s->off);
     if (s->xsrc) cudaFree(s->xsrc);
+    if (s->gsrc) cudaFree(s->gsrc);
+    if (s->gdst) cudaFree(s->gdst);
     if (s->order) cudaFree(s->order);
     if (s->counters) cudaFree(s->counters);
     delete s;
@@ -189,16 +273,21 @@ dwf_status tma_state_build(dwf_ctx* c) {
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
-    // offsets depend on K: fp64 table first, fp32 second
-    TmaTables t64 = build_tma_tables(12), t32 = build_tma_tables(6);
+    // fp64 tables first (K = 12, XOR-rotated lane order), fp32 second (K = 6, plain order)
+    TmaTables t64 = build_tma_tables_swz(12), t32 = build_tma_tables_plain(6);
     std::vector<uint16_t> off(t64.off);
     off.insert(off.end(), t32.off.begin(), t32.off.end());
+    const std::vector<uint16_t>& gdst = t64.gdst;
     std::vector<uint32_t> order = build_order(g, c->dhop_order, c->dhop_order_axes);
     DWF_CUDA_CHECK(c, cudaMalloc(&s->off, off.size() * sizeof(uint16_t)));
-    DWF_CUDA_CHECK(c, cudaMalloc(&s->xsrc, t64.xsrc.size()));
+    DWF_CUDA_CHECK(c, cudaMalloc(&s->xsrc, t32.xsrc.size()));
+    DWF_CUDA_CHECK(c, cudaMalloc(&s->gsrc, t64.gsrc.size()));
+    DWF_CUDA_CHECK(c, cudaMalloc(&s->gdst, gdst.size() * sizeof(uint16_t)));
     DWF_CUDA_CHECK(c, cudaMalloc(&s->order, order.size() * sizeof(uint32_t)));
     DWF_CUDA_CHECK(c, cudaMemcpy(s->off, off.data(), off.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
-    DWF_CUDA_CHECK(c, cudaMemcpy(s->xsrc, t64.xsrc.data(), t64.xsrc.size(), cudaMemcpyHostToDevice));
+    DWF_CUDA_CHECK(c, cudaMemcpy(s->xsrc, t32.xsrc.data(), t32.xsrc.size(), cudaMemcpyHostToDevice));
+    DWF_CUDA_CHECK(c, cudaMemcpy(s->gsrc, t64.gsrc.data(), t64.gsrc.size(), cudaMemcpyHostToDevice));
+    DWF_CUDA_CHECK(c, cudaMemcpy(s->gdst, gdst.data(), gdst.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
     DWF_CUDA_CHECK(c, cudaMemcpy(s->order, order.data(), order.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
     DWF_CUDA_CHECK(c, cudaMalloc(&s->counters, 4 * sizeof(int)));
     DWF_CUDA_CHECK(c, cudaMemset(s->counters, 0, 4 * sizeof(int)));
@@ -436,7 +525,9 @@ struct TmaArgs {
     void* out;
     const void* W;
     const uint16_t* off;      // [8][128]   (this output parity, this precision)
-    const uint8_t* xsrc;      // [2][32]    (this output parity)
+    const uint8_t* xsrc;      // [2][32]    fp32: x-face source lanes (this output parity)
+    const uint8_t* gsrc;      // [4][32]    fp64: gathered faces +x, -x, +y, -y: source lanes (this output parity)
+    const uint16_t* gdst;     // [4][32]    ... and stage offsets (this output parity, this precision)
     const uint32_t* order;    // [ntiles]
     int* counters;            // [3] queue / done / round-arrival counters
     EpiArgs epi;
@@ -458,8 +549,10 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
     constexpr int NCW = 4 * TPS;                       // consumer warps
     constexpr uint32_t REGION_BYTES = K * 512;
     constexpr uint32_t STAGE_BYTES = NREG * REGION_BYTES;
-    constexpr int REG_PROD = 24;
-    constexpr int REG_CONS = (TPS == 2) ? 240 : 232;
+    // setmaxnreg: the pool is the launch allocation, so (launch - PROD) x 128 must cover (CONS - launch) x consumers, or the
+    // consumers' setmaxnreg.inc blocks for ever.  fp64 (168 at launch, 256 consumers): 32 / 232; fp32 (128, 128): 24 / 232
+    constexpr int REG_PROD = (TPS == 2) ? 32 : 24;
+    constexpr int REG_CONS = 232;
 
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[2 * NST];   // full[NST], empty[NST]
@@ -489,29 +582,23 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
         reg_dec<REG_PROD>();
         if (warp != 0) return;
         const V* __restrict__ in = reinterpret_cast<const V*>(a.in);
-        const unsigned xs_p = a.xsrc[lane], xs_m = a.xsrc[32 + lane];
+        // gathered faces: this lane's source lane in the neighbour tile and its slot in the stage.
+        // fp64 (GATHER_Y): +x, -x, +y, -y faces into the conflict-free slots of build_tma_tables_swz;
+        // fp32: +x, -x faces into slot `lane` of regions 10, 11, the y faces come by TMA (build_tma_tables_plain)
+        constexpr bool GATHER_Y = (TPS == 2);
+        const uint32_t gs0 = GATHER_Y ? a.gsrc[lane] : a.xsrc[lane], gs1 = GATHER_Y ? a.gsrc[32 + lane] : a.xsrc[32 + lane];
+        const uint32_t gd0 = GATHER_Y ? (uint32_t)a.gdst[lane] * 16u : 10 * REGION_BYTES + lane * 16;
+        const uint32_t gd1 = GATHER_Y ? (uint32_t)a.gdst[32 + lane] * 16u : 11 * REGION_BYTES + lane * 16;
+        const uint32_t gs2 = GATHER_Y ? a.gsrc[64 + lane] : 0, gs3 = GATHER_Y ? a.gsrc[96 + lane] : 0;
+        const uint32_t gd2 = GATHER_Y ? (uint32_t)a.gdst[64 + lane] * 16u : 0, gd3 = GATHER_Y ? (uint32_t)a.gdst[96 + lane] * 16u : 0;
+        constexpr int NTMA = GATHER_Y ? 8 : 10;      // regions written by TMA boxes
         const uint32_t tile_vecs = (uint32_t)Ls * K * TSV;
         uint32_t n = 0, j = 0;
         int it = blockIdx.x;
-        // L2 policy of every read of the input field: its sectors are wanted again (as a neighbour's face or as the
-        // owner's slab), unlike the links and the output, which stream through once
-        const uint64_t pol = (a.l2hint == 1) ? l2_policy_evict_last() : (a.l2hint == 2 ? l2_policy_evict_first() : l2_policy_evict_normal());
         while (it < ntiles) {
             // next position in `order`: static round-robin, or the global in-order queue (tiles start in `order`
-            // sequence whatever the CTAs' speeds, which keeps neighbouring tiles in phase: their faces hit L2)
+            // sequence whatever the CTAs' speeds)
             int it_next = it + gridDim.x;
-            if (a.mode == 2 && j > 0) {
-                // lockstep rounds: every producer arrives, then waits until all have (CTAs are co-resident: grid =
-                // SMs x resident CTAs; the bounded spin makes a missing CTA cost time, never a hang).  Producers run
-                // up to NST slices ahead of their consumers, which hides the wait.
-                if (lane == 0) {
-                    atomicAdd(a.counters + 2, 1);
-                    const int target = (int)gridDim.x * (int)j;
-                    const long long t0 = clock64();
-                    while (*(volatile int*)(a.counters + 2) < target && clock64() - t0 < 4000000LL) __nanosleep(64);
-                }
-                __syncwarp();
-            }
             if (a.mode == 1) {
                 int v = 0;
                 if (lane == 0) v = atomicAdd(a.counters, 1) + (int)gridDim.x;
@@ -532,8 +619,9 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
             }
             if (lane == 0) next_of[j & 3] = tile_next;       // published by the release-arrive on slice 0's `full` barrier
             ++j;
-            const V* src_p = in + (size_t)nt[0] * tile_vecs + xs_p;
-            const V* src_m = in + (size_t)nt[1] * tile_vecs + xs_m;
+            // vector indices (< 2^31, checked at dwf_create) of this lane's face sources at s = 0
+            const uint32_t i0 = (uint32_t)nt[0] * tile_vecs + gs0, i1 = (uint32_t)nt[1] * tile_vecs + gs1;
+            const uint32_t i2 = (uint32_t)nt[2] * tile_vecs + gs2, i3 = (uint32_t)nt[3] * tile_vecs + gs3;
             for (int s = 0; s < Ls; ++s, ++n) {
                 const uint32_t st = n % NST, ph = (n / NST) & 1;
                 const uint32_t full = bar0 + 8 * st, empty = bar0 + 8 * (NST + st);
@@ -544,33 +632,35 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                     // later (issued a whole tile ahead they were evicted again before use and fetched twice)
                     if (s == Ls - 1 && tile_next >= 0)
                         l2_prefetch_bulk(reinterpret_cast<const V*>(a.W) + (size_t)tile_next * 8 * KG * TSV, 8 * KG * TSV * 16);
-                    const int nskip = __popc(a.skip & 0x3f0);
-                    mbar_arrive_expect_tx(full, (10 - nskip) * REGION_BYTES);
+                    const int nskip = __popc(a.skip & (GATHER_Y ? 0x0f0 : 0x3f0));
+                    mbar_arrive_expect_tx(full, (NTMA - nskip) * REGION_BYTES);
                     const int row_own = (tile * Ls + s) * K;
 #pragma unroll
-                    for (int tt = 0; tt < 4; ++tt) tma_load_3d_hint(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full, pol);
-                    if (!(a.skip & 0x010)) tma_load_3d_hint(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full, pol);
-                    if (!(a.skip & 0x020)) tma_load_3d_hint(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full, pol);
-                    if (!(a.skip & 0x040)) tma_load_4d_hint(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full, pol);
-                    if (!(a.skip & 0x080)) tma_load_4d_hint(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full, pol);
-                    if (!(a.skip & 0x100)) tma_load_4d_hint(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full, pol);
-                    if (!(a.skip & 0x200)) tma_load_4d_hint(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full, pol);
+                    for (int tt = 0; tt < 4; ++tt) tma_load_3d(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full);
+                    if (!(a.skip & 0x010)) tma_load_3d(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full);
+                    if (!(a.skip & 0x020)) tma_load_3d(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full);
+                    if (!(a.skip & 0x040)) tma_load_4d(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full);
+                    if (!(a.skip & 0x080)) tma_load_4d(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full);
+                    if (!GATHER_Y) {
+                        if (!(a.skip & 0x100)) tma_load_4d(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full);
+                        if (!(a.skip & 0x200)) tma_load_4d(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full);
+                    }
                 }
-                const V* sp = src_p + (size_t)s * (K * TSV);
-                const V* sm = src_m + (size_t)s * (K * TSV);
-                const uint32_t dp = base + 10 * REGION_BYTES + lane * 16, dm = base + 11 * REGION_BYTES + lane * 16;
+                const V* src = in + (size_t)s * (K * TSV);
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-                    if (!(a.skip & 0x400)) cp_async16_hint(dp + k * 512, sp + k * TSV, pol);
-                    if (!(a.skip & 0x800)) cp_async16_hint(dm + k * 512, sm + k * TSV, pol);
+                    if (!(a.skip & 0x400)) cp_async16_tma(base + gd0 + k * 512, src + i0 + k * TSV);
+                    if (!(a.skip & 0x800)) cp_async16_tma(base + gd1 + k * 512, src + i1 + k * TSV);
+                    if (GATHER_Y) {
+                        if (!(a.skip & 0x100)) cp_async16_tma(base + gd2 + k * 512, src + i2 + k * TSV);
+                        if (!(a.skip & 0x200)) cp_async16_tma(base + gd3 + k * 512, src + i3 + k * TSV);
+                    }
                 }
                 cp_async_mbar_arrive_noinc(full);
             }
             it = it_next;
         }
         if (a.mode != 0 && lane == 0) {          // the last CTA out re-arms the counters for the next launch
-            const uint32_t nrounds = ((uint32_t)ntiles + gridDim.x - 1) / gridDim.x;
-            if (a.mode == 2 && j < nrounds) atomicAdd(a.counters + 2, 1);     // no tile in the last round: arrive anyway
             __threadfence();
             if (atomicAdd(a.counters + 1, 1) == (int)gridDim.x - 1) {
                 atomicExch(a.counters, 0);
@@ -759,9 +849,11 @@ static dwf_status fill_args(dwf_ctx* c, TmaArgs& a, void* out, const void* in, i
     dwf_status st = get_maps(c, in, prec, maps);
     if (st != DWF_OK) return st;
     memset(&a, 0, sizeof(a));
-    a.g = c->g; a.in = in; a.out = out;
+    a.g = geom_prec(c, prec); a.in = in; a.out = out;
     a.W = (prec == DWF_F64) ? c->W64[out_parity] : c->W32[out_parity];
     a.off = s->off + (size_t)(prec == DWF_F64 ? 0 : 2 * 8 * TSV) + (size_t)out_parity * 8 * TSV;
+    a.gsrc = s->gsrc + (size_t)out_parity * 4 * 32;
+    a.gdst = s->gdst + (size_t)out_parity * 4 * 32;
     a.xsrc = s->xsrc + (size_t)out_parity * 2 * 32;
     a.order = s->order;
     a.counters = s->counters;

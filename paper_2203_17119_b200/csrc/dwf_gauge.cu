@@ -51,9 +51,9 @@ dwf_status launch_gauge_prep(dwf_ctx* c, const double* Ucanon) {
     const int block = 128, grid = (g.Vh * 8 + block - 1) / block;
     for (int par = 0; par < 2; ++par) {
         const int kg64 = (ng + 1) / 2 * 2, kg32 = (ng + 3) / 4 * 4;
-        gauge_prep_kernel<double><<<grid, block, 0, c->stream>>>(g, Ucanon, (double*)c->W64[par], par, ng, kg64, 2,
+        gauge_prep_kernel<double><<<grid, block, 0, c->stream>>>(geom_prec(c, DWF_F64), Ucanon, (double*)c->W64[par], par, ng, kg64, 2,
                                                                  c->cut[0], c->cut[1], c->cut[2], c->cut[3]);
-        gauge_prep_kernel<float><<<grid, block, 0, c->stream>>>(g, Ucanon, (float*)c->W32[par], par, ng, kg32, 4,
+        gauge_prep_kernel<float><<<grid, block, 0, c->stream>>>(geom_prec(c, DWF_F32), Ucanon, (float*)c->W32[par], par, ng, kg32, 4,
                                                                 c->cut[0], c->cut[1], c->cut[2], c->cut[3]);
         c->launches += 2;
     }
@@ -91,7 +91,7 @@ __global__ void pack_kernel(Geom g, R* __restrict__ native, R* __restrict__ cano
 }
 
 dwf_status launch_pack(dwf_ctx* c, void* native, const void* canon, int prec, int parity, bool unpack) {
-    const Geom& g = c->g;
+    const Geom g = geom_prec(c, prec);
     const long long n = (long long)g.Vh * g.Ls;
     const int block = 128;
     const int grid = (int)((n + block - 1) / block);
@@ -115,7 +115,7 @@ dwf_status launch_pack(dwf_ctx* c, void* native, const void* canon, int prec, in
 
 // native -> native with a precision change; ACCUM: dst += src (used for x64 += e32)
 template <typename RD, typename RS, bool ACCUM>
-__global__ void convert_kernel(Geom g, RD* __restrict__ dst, const RS* __restrict__ src) {
+__global__ void convert_kernel(Geom g, RD* __restrict__ dst, const RS* __restrict__ src, int swz_d, int swz_s) {
     // one thread per (tile, s, lane, group of 4 reals)
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const long long n = (long long)g.Vh * g.Ls * 6;
@@ -128,8 +128,10 @@ __global__ void convert_kernel(Geom g, RD* __restrict__ dst, const RS* __restric
     const int tile = (int)(r / g.Ls);
 #pragma unroll
     for (int j = 0; j < 4; ++j) {
-        const size_t si = native_real_index<RS>(g, tile, lane, s, q * 4 + j);
-        const size_t di = native_real_index<RD>(g, tile, lane, s, q * 4 + j);
+        // `lane` is the plain-order lane; a field in the XOR-rotated order (4^4 tiles) holds that site at lane ^ (tz << 1)
+        const int rot = ((lane >> 3) & 3) << 1;
+        const size_t si = native_real_index<RS>(g, tile, swz_s ? (lane ^ rot) : lane, s, q * 4 + j);
+        const size_t di = native_real_index<RD>(g, tile, swz_d ? (lane ^ rot) : lane, s, q * 4 + j);
         if (ACCUM) dst[di] += (RD)src[si]; else dst[di] = (RD)src[si];
     }
 }
@@ -143,13 +145,13 @@ dwf_status launch_convert(dwf_ctx* c, void* dst, int dprec, const void* src, int
         void* d = (char*)dst + h * half_bytes(g, dprec);
         const void* s = (const char*)src + h * half_bytes(g, sprec);
         if (dprec == DWF_F32 && sprec == DWF_F64)
-            convert_kernel<float, double, false><<<grid, block, 0, c->stream>>>(g, (float*)d, (const double*)s);
+            convert_kernel<float, double, false><<<grid, block, 0, c->stream>>>(g, (float*)d, (const double*)s, 0, c->swz64);
         else if (dprec == DWF_F64 && sprec == DWF_F32)
-            convert_kernel<double, float, false><<<grid, block, 0, c->stream>>>(g, (double*)d, (const float*)s);
+            convert_kernel<double, float, false><<<grid, block, 0, c->stream>>>(g, (double*)d, (const float*)s, c->swz64, 0);
         else if (dprec == DWF_F64)
-            convert_kernel<double, double, false><<<grid, block, 0, c->stream>>>(g, (double*)d, (const double*)s);
+            convert_kernel<double, double, false><<<grid, block, 0, c->stream>>>(g, (double*)d, (const double*)s, 0, 0);
         else
-            convert_kernel<float, float, false><<<grid, block, 0, c->stream>>>(g, (float*)d, (const float*)s);
+            convert_kernel<float, float, false><<<grid, block, 0, c->stream>>>(g, (float*)d, (const float*)s, 0, 0);
         c->launches++;
     }
     DWF_CUDA_CHECK(c, cudaGetLastError());
@@ -161,7 +163,7 @@ dwf_status launch_add_f32_to_f64(dwf_ctx* c, void* x64, const void* e32, size_t)
     const long long n = (long long)g.Vh * g.Ls * 6;
     const int block = 256;
     const int grid = (int)((n + block - 1) / block);
-    convert_kernel<double, float, true><<<grid, block, 0, c->stream>>>(g, (double*)x64, (const float*)e32);
+    convert_kernel<double, float, true><<<grid, block, 0, c->stream>>>(g, (double*)x64, (const float*)e32, c->swz64, 0);
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
     return DWF_OK;

@@ -27,6 +27,7 @@ struct Geom {
     int Vh;      // sites of one parity  (= ntiles*TS)
     int Ls;
     int antiperiodic_t;
+    int swz;     // lane order: y rows XOR-rotated by tz (dwf_layout.cuh); set per precision by geom_prec()
 };
 
 // 5-D coefficient tables: out_s = sum_s' Tp[s][s'] in_s' on P+ components (spin 0,1), Tm on P- (spin 2,3)
@@ -66,9 +67,10 @@ struct dwf_ctx {
     int dhop_order_axes = 0;   // blob path, fastest-first axis digits
     void* tma = nullptr;   // dwf::TmaState (dwf_dhop_tma.cu), built at dwf_set_gauge for 4^4 tiles
     // tables of the pipelined Dhop kernel (dwf_dhop_pipe.cu), built at dwf_set_gauge
-    uint16_t* pipe_nbslot = nullptr;
-    int16_t* pipe_slot_dir = nullptr;
-    uint16_t* pipe_slot_lane = nullptr;
+    uint16_t* pipe_nbslot[2] = {nullptr, nullptr};      // [precision]: the two precisions differ in lane order
+    int16_t* pipe_slot_dir[2] = {nullptr, nullptr};
+    uint16_t* pipe_slot_lane[2] = {nullptr, nullptr};
+    int swz64 = 0;         // fp64 native fields use the XOR-rotated lane order (4^4 tiles); fp32 fields never do
     int pipe_nslot = 0;
     double inner_tol = 1e-4;
     int max_restarts = 20;
@@ -104,6 +106,15 @@ struct dwf_ctx {
 };
 
 namespace dwf {
+
+// geometry as seen by fields of one precision: fp64 fields of 4^4 tiles are stored in the XOR-rotated lane order that makes
+// the fp64 Dhop kernel's shared-memory accesses conflict-free; fp32 fields keep the plain order (its kernel has no
+// registers left for the extra face gathers that order needs).  dwf_convert and x64 += e32 permute the lanes.
+inline Geom geom_prec(const dwf_ctx* c, int prec) {
+    Geom g = c->g;
+    g.swz = (prec == DWF_F64) ? c->swz64 : 0;
+    return g;
+}
 
 inline size_t half_vecs(const Geom& g, int prec) { return (size_t)g.Vh * g.Ls * (prec == DWF_F64 ? 12 : 6); }
 inline size_t half_bytes(const Geom& g, int prec) { return half_vecs(g, prec) * 16; }
