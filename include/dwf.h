@@ -84,8 +84,7 @@ dwf_status dwf_destroy(dwf_ctx* ctx);
  *   kernels where the TMA Dhop kernel applies (4^4 tiles, 2-row links); get "fused_active" tells whether they do
  *   "dhop_kernel" 0 auto / 1 shape-generic / 2 cp.async tile kernel, "dhop_grid" CTAs of the persistent TMA kernel,
  *   "dhop_order" / "dhop_order_axes" tile traversal (blob extents / path axes as decimal digits),
- *   "dhop_dynamic" 0 static round-robin / 1 global in-order queue / 2 lockstep rounds, "dhop_l2hint" 0/1/2
- *   (normal / evict_last / evict_first on input reads): tuning, any time.  "dhop_skip" is a measurement aid
+ *   "dhop_dynamic" 0 static round-robin / 1 global in-order queue: tuning, any time.  "dhop_skip" is a measurement aid
  *   (bit r: halo region r is not loaded; results are then WRONG) and must stay 0 otherwise. */
 dwf_status dwf_set_option(dwf_ctx* ctx, const char* key, double val);
 dwf_status dwf_get_option(const dwf_ctx* ctx, const char* key, double* val);

@@ -408,8 +408,7 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
     }
     else if (k == "fuse") c->fuse = (val != 0.0);
     else if (k == "dhop_skip") c->dhop_skip = (int)val;
-    else if (k == "dhop_l2hint") { if (val < 0 || val > 2) return DWF_EINVAL; c->dhop_l2hint = (int)val; }
-    else if (k == "dhop_dynamic") { if (val < 0 || val > 2) return DWF_EINVAL; c->dhop_dynamic = (int)val; }
+    else if (k == "dhop_dynamic") { if (val < 0 || val > 1) return DWF_EINVAL; c->dhop_dynamic = (int)val; }
     else if (k == "dhop_nst") { if (val != 2 && val != 3) return DWF_EINVAL; c->dhop_nst = (int)val; }
     else if (k == "time_dhop") {       // (re)start per-launch event timing of the Dhop kernel
         DWF_TRY(dhop_timing_flush(c));
@@ -446,7 +445,6 @@ dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
     else if (k == "dhop_nst") *val = c->dhop_nst;
     else if (k == "dhop_grid") *val = c->dhop_grid;
     else if (k == "dhop_dynamic") *val = c->dhop_dynamic;
-    else if (k == "dhop_l2hint") *val = c->dhop_l2hint;
     else if (k == "fuse") *val = c->fuse;
     else if (k == "fused_active") *val = dhop_fused_available(c) ? 1.0 : 0.0;
     else if (k == "dhop_order") *val = c->dhop_order;

@@ -60,9 +60,8 @@ struct dwf_ctx {
     int dhop_nst = 3;      // ring depth of the pipelined fp32 kernel
     int dhop_grid = 0;     // CTAs of the persistent TMA kernel (0 = SMs x resident CTAs)
     int fuse = 1;          // Mpc / CG through the Dhop kernel's fused 5-D epilogues when the TMA kernel applies (0: separate op5 kernels)
-    int dhop_dynamic = 1;  // TMA kernel tile scheduling: 0 static round-robin, 1 global in-order queue (default; the fused launches, which reduce, always use 0), 2 static rounds in lockstep
+    int dhop_dynamic = 1;  // TMA kernel tile scheduling: 1 global in-order queue (default), 0 static round-robin (always used by the fused launches, which reduce)
     int dhop_skip = 0;     // debug only (traffic attribution): halo regions the TMA kernel does not load
-    int dhop_l2hint = 0;   // L2 eviction priority of the TMA kernel's input-field reads: 0 normal, 1 evict_last, 2 evict_first
     int dhop_order = 0;    // tile traversal of the TMA kernel: blob extents in tiles as digits (0 = default), dwf_dhop_tma.cu
     int dhop_order_axes = 0;   // blob path, fastest-first axis digits
     void* tma = nullptr;   // dwf::TmaState (dwf_dhop_tma.cu), built at dwf_set_gauge for 4^4 tiles

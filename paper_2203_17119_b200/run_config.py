@@ -73,10 +73,40 @@ def run(cfg, U, b_np, with_sweeps=True, max_iter=50000, extras=False):
     return rep
 
 
+def roofline_sweep(cfg, U, hbm_gbs):
+    """SURVEY 8(d) / BASELINE configs[3]: Dhop and Mpc^dag Mpc over links in {12, 18} reals x Ls in {8, 12, 16} x {fp32, fp64},
+    half-volume (EO) and full-volume Dhop.  Algorithmic bytes per 5-D site: 48 B + 8 g B / Ls (B = 4 or 8)."""
+    A = api
+    rows = []
+    for ng in (12, 18):
+        for Ls in (8, 12, 16):
+            c = dataclasses.replace(cfg, Ls=Ls)
+            g = api.from_config(c, compress12=int(ng == 12))
+            g.set_gauge(U)
+            n5h = (c.V4 // 2) * Ls
+            for prec, name, B in ((A.F32, "f32", 4), (A.F64, "f64", 8)):
+                src = g.new_native(prec, A.FULL).normal_()
+                dst = g.new_native(prec, A.FULL)
+                h = src.numel() // 2
+                ms_eo = _time(lambda: g.dhop(src[:h], A.ODD, False, prec, out=dst[h:]), 20)
+                ms_full = _time(lambda: g.dhop(src, A.FULL, False, prec, out=dst), 10)
+                ms_mm = _time(lambda: g.mdagm(src[:h], prec, out=dst[:h]), 5)
+                by = n5h * 48 * B + (c.V4 // 2) * 8 * ng * B
+                rows.append({"links": ng, "Ls": Ls, "prec": name, "dhop_eo_ms": ms_eo, "dhop_full_ms": ms_full,
+                             "dhop_eo_frac_hbm": by / ms_eo / 1e6 / hbm_gbs, "dhop_full_frac_hbm": 2 * by / ms_full / 1e6 / hbm_gbs,
+                             "dhop_full_gflops": FLOP_DHOP * 2 * n5h / ms_full / 1e6, "mdagm_ms": ms_mm,
+                             "mdagm_gflops": 2 * FLOP_MPC * n5h / ms_mm / 1e6, "fused": bool(g.get_option("fused_active"))})
+                del src, dst
+            g.close()
+    return rows
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("config", choices=sorted(inputs.CONFIGS))
     ap.add_argument("--no-uncut", action="store_true", help="cut configurations: skip the uncut comparison solve")
+    ap.add_argument("--sweep", action="store_true", help="only the Dhop / Mpc^dag Mpc roofline sweep (links x Ls x precision)")
+    ap.add_argument("--hbm-gbs", type=float, default=6448.1, help="HBM roofline for --sweep (MEASURED_PEAKS.json hbm_gbs)")
     ap.add_argument("--extras", action="store_true", help="also time the multishift CG (4 shifts) and a 16th-order Chebyshev filter")
     args = ap.parse_args()
     if not torch.cuda.is_available():
@@ -87,6 +117,10 @@ def main():
     b = inputs.source_half(cfg.dims, cfg.Ls, cfg.source_seed, parity=1)
     out = {"config": cfg.name, "params": {"M5": cfg.M5, "mf": cfg.mf, "b5": cfg.b5, "c5": cfg.c5, "gauge": cfg.gauge, "eps": cfg.eps},
            "plaquette": inputs.plaquette(U), "input_seconds": time.perf_counter() - t0}
+    if args.sweep:
+        out["roofline_sweep"] = roofline_sweep(cfg, U, args.hbm_gbs)
+        print(json.dumps(out), flush=True)
+        return
     out["as_configured"] = run(cfg, U, b, extras=args.extras)
     if any(cfg.cut) and not args.no_uncut:
         out["uncut_operator"] = run(dataclasses.replace(cfg, cut=(0, 0, 0, 0)), U, b, with_sweeps=False)
