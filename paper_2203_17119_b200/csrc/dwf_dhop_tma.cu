@@ -42,25 +42,44 @@ struct TmaTables {
     std::vector<uint16_t> off;     // [2][8][128]  stage offset (16-byte units, k = 0) of the leg's neighbour
     std::vector<uint8_t> gsrc;     // [2][4][32]   gathered faces (+x, -x, +y, -y): source lane in the neighbour tile
     std::vector<uint16_t> gdst;    // [2][4][32]   ... and its stage offset (16-byte units, k = 0)
-    std::vector<uint8_t> xsrc;     // [2][2][32]   plain order (fp32): source lane (in the +x / -x tile) of each x-face slot
+    std::vector<uint8_t> xsrc;     // [2][2][32]   plain order (fp32): source lane (in the +x / -x tile) of each x-face site
+    std::vector<uint16_t> xdst;    // [2][2][32]   ... and its stage offset (16-byte units, k = 0)
 };
 
 inline int lane_of_plain(int tx, int ty, int tz, int tt) { return ((tt * 4 + tz) * 4 + ty) * 2 + (tx >> 1); }
 
-// fp32 fields: plain lane order, +-y faces by TMA boxes, +-x faces gathered (the kernel has no registers for more)
+// fp32 fields: plain lane order, +-y faces by TMA boxes, +-x faces gathered (the kernel has no registers for more).
+// The gathered x faces are interleaved over regions 10 and 11 like in the fp64 scheme below (+x sites on the even bank
+// groups 2 ty, -x sites on the odd ones 2 ty + 1: the groups the quarter warp's interior lanes leave free), which removes
+// the x-leg bank conflicts; the y legs keep theirs (their faces are TMA boxes with a fixed layout).
 TmaTables build_tma_tables_plain(int K) {
     TmaTables t;
     t.off.assign(2 * 8 * TSV, 0);
     t.xsrc.assign(2 * 2 * 32, 0);
+    t.xdst.assign(2 * 2 * 32, 0);
     for (int p = 0; p < 2; ++p) {
         const int q = 1 - p;   // input parity
+        int xslot[2][4][4][4];     // [f][tt][tz][ty] stage offset of the x-face site, f = 0: +x tile (tx = 0), 1: -x tile (tx = 3)
+        int cnt[2][8], nface[2] = {0, 0};
+        memset(cnt, 0, sizeof(cnt));
+        for (int f = 0; f < 2; ++f)
+            for (int tt = 0; tt < 4; ++tt)
+                for (int tz = 0; tz < 4; ++tz)
+                    for (int ty = 0; ty < 4; ++ty) {
+                        xslot[f][tt][tz][ty] = -1;
+                        const int tx = f ? 3 : 0;
+                        if (((q + tx + ty + tz + tt) & 1) != 0) continue;
+                        const int b = 2 * ty + f;
+                        const int s64 = b + 8 * cnt[f][b]++;
+                        const int o = (10 + (s64 >> 5)) * K * 32 + (s64 & 31);
+                        xslot[f][tt][tz][ty] = o;
+                        const int i = nface[f]++;
+                        t.xsrc[(p * 2 + f) * 32 + i] = (uint8_t)lane_of_plain(tx, ty, tz, tt);
+                        t.xdst[(p * 2 + f) * 32 + i] = (uint16_t)o;
+                    }
         for (int tt = 0; tt < 4; ++tt)
             for (int tz = 0; tz < 4; ++tz)
-                for (int ty = 0; ty < 4; ++ty) {
-                    const int row = (tt * 4 + tz) * 4 + ty;
-                    // x-face slots: row >> 1 enumerates the rows of the needed parity (ty alternates inside (tz,tt))
-                    if (((q + ty + tz + tt) & 1) == 0) t.xsrc[(p * 2 + 0) * 32 + (row >> 1)] = (uint8_t)(row * 2 + 0);   // +x tile, tx = 0
-                    else                               t.xsrc[(p * 2 + 1) * 32 + (row >> 1)] = (uint8_t)(row * 2 + 1);   // -x tile, tx = 3
+                for (int ty = 0; ty < 4; ++ty)
                     for (int txh = 0; txh < 2; ++txh) {
                         const int tx = 2 * txh + ((p + ty + tz + tt) & 1);
                         const int lane = lane_of_plain(tx, ty, tz, tt);
@@ -68,27 +87,24 @@ TmaTables build_tma_tables_plain(int K) {
                             const int mu = leg >> 1;
                             int y[4] = {tx, ty, tz, tt};
                             y[mu] += (leg & 1) ? -1 : +1;
-                            int region, slot;
+                            int o;
                             if (y[mu] >= 0 && y[mu] < 4) {
-                                region = y[3];
-                                slot = (y[2] * 4 + y[1]) * 2 + (y[0] >> 1);
+                                o = y[3] * K * 32 + (y[2] * 4 + y[1]) * 2 + (y[0] >> 1);
                             } else {
                                 const int up = (y[mu] >= 4);
                                 y[mu] = (y[mu] + 4) & 3;
                                 const int yh = y[0] >> 1;
-                                if (mu == 3)      { region = up ? 4 : 5;   slot = (y[2] * 4 + y[1]) * 2 + yh; }
-                                else if (mu == 2) { region = up ? 6 : 7;   slot = y[3] * 8 + y[1] * 2 + yh; }
-                                else if (mu == 1) { region = up ? 8 : 9;   slot = (y[3] * 4 + y[2]) * 2 + yh; }
-                                else              { region = up ? 10 : 11; slot = ((y[3] * 4 + y[2]) * 4 + y[1]) >> 1; }
+                                if (mu == 3)      o = (up ? 4 : 5) * K * 32 + (y[2] * 4 + y[1]) * 2 + yh;
+                                else if (mu == 2) o = (up ? 6 : 7) * K * 32 + y[3] * 8 + y[1] * 2 + yh;
+                                else if (mu == 1) o = (up ? 8 : 9) * K * 32 + (y[3] * 4 + y[2]) * 2 + yh;
+                                else              o = xslot[up ? 0 : 1][y[3]][y[2]][y[1]];
                             }
-                            t.off[(p * 8 + leg) * TSV + lane] = (uint16_t)(region * K * 32 + slot);
+                            t.off[(p * 8 + leg) * TSV + lane] = (uint16_t)o;
                         }
                     }
-                }
     }
     return t;
 }
-
 
 // lane order of dwf_layout.cuh for 4^4 tiles: y rows XOR-rotated by tz
 inline int lane_of(int tx, int ty, int tz, int tt) { return ((tt * 4 + tz) * 4 + (ty ^ tz)) * 2 + (tx >> 1); }
@@ -237,6 +253,7 @@ EncodeTiledFn encode_fn() {
 struct TmaState {
     uint16_t* off = nullptr;      // device [2][8][128]
     uint8_t* xsrc = nullptr;      // device [2][2][32]   (fp32 path)
+    uint16_t* xdst = nullptr;     // device [2][2][32]   (fp32 path)
     uint8_t* gsrc = nullptr;      // device [2][4][32]   (fp64 path)
     uint16_t* gdst = nullptr;     // device [2][4][32]   (fp64 path)
     uint32_t* order = nullptr;    // device [ntiles]
@@ -252,6 +269,7 @@ void tma_state_free(dwf_ctx* c) {
     if (!s) return;
     if (s->off) cudaFree(s->off);
     if (s->xsrc) cudaFree(s->xsrc);
+    if (s->xdst) cudaFree(s->xdst);
     if (s->gsrc) cudaFree(s->gsrc);
     if (s->gdst) cudaFree(s->gdst);
     if (s->order) cudaFree(s->order);
@@ -281,11 +299,13 @@ dwf_status tma_state_build(dwf_ctx* c) {
     std::vector<uint32_t> order = build_order(g, c->dhop_order, c->dhop_order_axes);
     DWF_CUDA_CHECK(c, cudaMalloc(&s->off, off.size() * sizeof(uint16_t)));
     DWF_CUDA_CHECK(c, cudaMalloc(&s->xsrc, t32.xsrc.size()));
+    DWF_CUDA_CHECK(c, cudaMalloc(&s->xdst, t32.xdst.size() * sizeof(uint16_t)));
     DWF_CUDA_CHECK(c, cudaMalloc(&s->gsrc, t64.gsrc.size()));
     DWF_CUDA_CHECK(c, cudaMalloc(&s->gdst, gdst.size() * sizeof(uint16_t)));
     DWF_CUDA_CHECK(c, cudaMalloc(&s->order, order.size() * sizeof(uint32_t)));
     DWF_CUDA_CHECK(c, cudaMemcpy(s->off, off.data(), off.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
     DWF_CUDA_CHECK(c, cudaMemcpy(s->xsrc, t32.xsrc.data(), t32.xsrc.size(), cudaMemcpyHostToDevice));
+    DWF_CUDA_CHECK(c, cudaMemcpy(s->xdst, t32.xdst.data(), t32.xdst.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
     DWF_CUDA_CHECK(c, cudaMemcpy(s->gsrc, t64.gsrc.data(), t64.gsrc.size(), cudaMemcpyHostToDevice));
     DWF_CUDA_CHECK(c, cudaMemcpy(s->gdst, gdst.data(), gdst.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
     DWF_CUDA_CHECK(c, cudaMemcpy(s->order, order.data(), order.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
@@ -484,6 +504,7 @@ struct TmaArgs {
     const void* W;
     const uint16_t* off;      // [8][128]   (this output parity, this precision)
     const uint8_t* xsrc;      // [2][32]    fp32: x-face source lanes (this output parity)
+    const uint16_t* xdst;     // [2][32]    fp32: ... and stage offsets
     const uint8_t* gsrc;      // [4][32]    fp64: gathered faces +x, -x, +y, -y: source lanes (this output parity)
     const uint16_t* gdst;     // [4][32]    ... and stage offsets (this output parity, this precision)
     const uint32_t* order;    // [ntiles]
@@ -513,6 +534,7 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
 
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[2 * NST];   // full[NST], empty[NST]
+    __shared__ double wsum[2][4 * TPS];   // per-tile |.|^2 partials of the consumer warps (fused epilogue), double-buffered
     __shared__ int next_of[4];     // slot j & 3, written before slice 0 of this CTA's j-th tile: the tile it takes after it (-1: none)
 
     const Geom& g = a.g;
@@ -541,11 +563,11 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
         const V* __restrict__ in = reinterpret_cast<const V*>(a.in);
         // gathered faces: this lane's source lane in the neighbour tile and its slot in the stage.
         // fp64 (GATHER_Y): +x, -x, +y, -y faces into the conflict-free slots of build_tma_tables_swz;
-        // fp32: +x, -x faces into slot `lane` of regions 10, 11, the y faces come by TMA (build_tma_tables_plain)
+        // fp32: +x, -x faces interleaved over regions 10, 11, the y faces come by TMA (build_tma_tables_plain)
         constexpr bool GATHER_Y = (TPS == 2);
         const uint32_t gs0 = GATHER_Y ? a.gsrc[lane] : a.xsrc[lane], gs1 = GATHER_Y ? a.gsrc[32 + lane] : a.xsrc[32 + lane];
-        const uint32_t gd0 = GATHER_Y ? (uint32_t)a.gdst[lane] * 16u : 10 * REGION_BYTES + lane * 16;
-        const uint32_t gd1 = GATHER_Y ? (uint32_t)a.gdst[32 + lane] * 16u : 11 * REGION_BYTES + lane * 16;
+        const uint32_t gd0 = (uint32_t)(GATHER_Y ? a.gdst[lane] : a.xdst[lane]) * 16u;
+        const uint32_t gd1 = (uint32_t)(GATHER_Y ? a.gdst[32 + lane] : a.xdst[32 + lane]) * 16u;
         const uint32_t gs2 = GATHER_Y ? a.gsrc[64 + lane] : 0, gs3 = GATHER_Y ? a.gsrc[96 + lane] : 0;
         const uint32_t gd2 = GATHER_Y ? (uint32_t)a.gdst[64 + lane] * 16u : 0, gd3 = GATHER_Y ? (uint32_t)a.gdst[96 + lane] * 16u : 0;
         constexpr int NTMA = GATHER_Y ? 8 : 10;      // regions written by TMA boxes
@@ -759,22 +781,25 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                 }
             }
         }
+        if constexpr (EPI != 0) {
+            // |out|^2 of this tile: fixed-tree sum over the consumer threads into partials[tile] -- independent of which
+            // CTA took the tile, so the reduction is bit-reproducible under the dynamic tile queue as well
+            if (a.epi.partials != nullptr) {
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
+                if (lane == 0) wsum[j & 1][cw] = nrm;
+                asm volatile("bar.sync 1, %0;" ::"n"(128 * TPS) : "memory");
+                if (ctid == 0) {
+                    double t = 0.0;
+#pragma unroll
+                    for (int i = 0; i < NCW; ++i) t += wsum[j & 1][i];
+                    a.epi.partials[tile] = t;
+                }
+                nrm = 0.0;
+            }
+        }
         tile = tile_next;
         ++j;
-    }
-    if (EPI != 0 && a.epi.partials != nullptr) {
-        // fixed-tree sum over the consumer threads (static tile assignment: bit-reproducible run to run)
-        __shared__ double wsum[NCW];
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
-        if (lane == 0) wsum[cw] = nrm;
-        asm volatile("bar.sync 1, %0;" ::"n"(128 * TPS) : "memory");
-        if (ctid == 0) {
-            double t = 0.0;
-#pragma unroll
-            for (int i = 0; i < NCW; ++i) t += wsum[i];
-            a.epi.partials[blockIdx.x] = t;
-        }
     }
 }
 
@@ -812,6 +837,7 @@ static dwf_status fill_args(dwf_ctx* c, TmaArgs& a, void* out, const void* in, i
     a.gsrc = s->gsrc + (size_t)out_parity * 4 * 32;
     a.gdst = s->gdst + (size_t)out_parity * 4 * 32;
     a.xsrc = s->xsrc + (size_t)out_parity * 2 * 32;
+    a.xdst = s->xdst + (size_t)out_parity * 2 * 32;
     a.order = s->order;
     a.counters = s->counters;
     a.mode = c->dhop_dynamic;
@@ -852,11 +878,9 @@ dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_pari
     e.mode = EPI_FINAL;
     e.xin = xin;
     e.bee = bee; e.mcee = -cee; e.mf = c->mf; e.scale = scale;
-    a.mode = 0;                                    // static tile assignment: reproducible reductions
     int grid = 0;
     if (norm_slot >= 0) {
-        TmaState* s = (TmaState*)c->tma;
-        st = ensure_partials(c, std::max(s->num_sms * 2, c->dhop_grid));
+        st = ensure_partials(c, c->g.ntiles);              // one partial per tile
         if (st != DWF_OK) return st;
         e.partials = c->partials;
     }
@@ -869,7 +893,7 @@ dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_pari
     const double B = (prec == DWF_F64) ? 8.0 : 4.0;
     st = dhop_time_end(c, 3.0 * (double)half_bytes(c->g, prec) + (double)c->g.Vh * 8 * 12 * B);
     if (st != DWF_OK) return st;
-    if (norm_slot >= 0) return launch_reduce(c, grid, norm_slot);
+    if (norm_slot >= 0) return launch_reduce(c, c->g.ntiles, norm_slot);
     return DWF_OK;
 }
 
