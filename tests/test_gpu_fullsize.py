@@ -121,3 +121,19 @@ def test_c3_mixed_precision_cg_to_1e10(c3):
     true_res = np.sqrt(orc.norm2(odd - orc.mdagm(xs)) / orc.norm2(odd))      # the oracle recomputes it
     assert true_res <= cfg.tol * (1 + 1e-6)
     assert abs(true_res - info["resid_true"]) <= 1e-6 * true_res + 1e-16
+
+
+def test_c4_results_are_bit_reproducible_and_schedule_independent(c4):
+    """every tile is computed by one CTA in a fixed order and the |.|^2 sums are fixed-tree per tile, so the
+    operators and the CG scalars must not depend on the run or on the tile scheduling (global queue vs static round-robin)."""
+    import torch
+    A, g, odd = c4["api"], c4["g"], c4["odd"]
+    nat = g.pack(odd, A.F64, A.ODD)
+    ref = g.mdagm(nat, A.F64)
+    _, info_ref, _ = g.cg(nat, 1e-30, 3, A.CG_F64)
+    for dyn in (1, 0, 1):
+        g.set_option("dhop_dynamic", dyn)
+        assert torch.equal(g.mdagm(nat, A.F64), ref)
+        _, info, _ = g.cg(nat, 1e-30, 3, A.CG_F64)
+        assert info["resid_iter"] == info_ref["resid_iter"] and info["resid_true"] == info_ref["resid_true"]
+    g.set_option("dhop_dynamic", 1)
