@@ -224,9 +224,12 @@ def run_dwf(args, cfg):
     dhop_bytes = dhop_bytes_total / max(dhop_n, 1)
     achieved = dhop_bytes / (dhop_avg_ms * 1e-3) / 1e9
     traffic = None
-    tp = os.path.join(ROOT, "profiles", "dhop_traffic.json")
+    tp = os.path.join(ROOT, "profiles", "dhop_traffic.csv")       # ncu DRAM bytes per launch (profiles/r01d_dhop.md)
     if os.path.exists(tp):
-        traffic = json.load(open(tp)).get("dhop_f64_dram_bytes_per_launch")
+        import csv
+        for row in csv.DictReader(open(tp)):
+            if row["kernel"] == "dhop_f64":
+                traffic = float(row["dram_bytes_per_launch"])
     roofline = {"bound": "hbm", "kernel": "dhop_tma_kernel<double> (half-volume, 12-real links; per CG iteration 3 plain launches + 1 with the fused Mee epilogue)",
                 "achieved": achieved, "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / hbm_peak,
                 "traffic": traffic, "algorithmic_bytes_per_launch": dhop_bytes, "avg_launch_ms": dhop_avg_ms,
