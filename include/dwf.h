@@ -141,6 +141,19 @@ dwf_status dwf_multishift_cg(dwf_ctx* ctx, void* x_dev, const void* b_dev, const
  * A = Mpc^dag Mpc, by t_0 = in, t_1 = a in, t_{k+1} = 2 a t_k - t_{k-1}.  Native ODD fields of precision prec, device
  * pointers, out != in; hi > lo; order >= 0.  Enqueued on the context stream (no synchronisation). */
 dwf_status dwf_chebyshev(dwf_ctx* ctx, void* out_dev, const void* in_dev, double lo, double hi, int order, dwf_prec prec);
+/* Domain decomposition objects of the paper.  They need a Dirichlet cut with an EVEN number of blocks
+ * in every cut direction (else DWF_EINVAL); dwf_set_gauge then also keeps the links without the cut.
+ * Omega = sites whose block indices floor(x_mu / B_mu), summed over the cut directions, are even (eqs. 1-2).
+ * dwf_domain_project: out = P in on FULL native fields (out may alias in), which = 0: P_Omega, 1: P_Omegabar, 2: the
+ *   boundary projector P_dbar of eq. 8, found by mask-and-shift: sites of Omega with a cut
+ *   link, times (1 +- gamma_mu)/2 for Shamir sites on one cut face, times 1 otherwise (reading in DESIGN.md section 2).
+ * dwf_boundary_op: FULL fp64 native fields, out != in.  inverse = 0: R phi = P phi - P D_O^-1 D_d D_Ob^-1 D_dbar phi (eq. 13,
+ *   PAPER.md:107-109; two Dirichlet solves); inverse != 0: R^-1 phi = P phi - P D^-1 D_dbar_hat phi (eq. 14, PAPER.md:111-113;
+ *   one solve with the uncut operator).  Solves as dwf_solve (tol, max_iter, mode); info->iters_total sums them,
+ *   info->resid_full is the worst |eta - M psi|/|eta|.  Synchronises. */
+dwf_status dwf_domain_project(dwf_ctx* ctx, void* out_dev, const void* in_dev, int which, dwf_prec prec);
+dwf_status dwf_boundary_op(dwf_ctx* ctx, void* out_dev, const void* in_dev, int inverse, double tol, int max_iter,
+                           dwf_cg_mode mode, dwf_cg_info* info);
 /* M psi = eta on FULL fp64 native fields through the red-black wrap (reading C6):
  * eta' = eta_o - Moe Mee^-1 eta_e; Mpc^dag Mpc psi_o = Mpc^dag eta'; psi_e = Mee^-1 (eta_e - Meo psi_o). */
 dwf_status dwf_solve(dwf_ctx* ctx, void* psi_dev, const void* eta_dev, double tol, int max_iter, dwf_cg_mode mode,

@@ -27,7 +27,7 @@ OK, EINVAL, ENOMEM, ECUDA, ESTATE, ENOTCONV = 0, 1, 2, 3, 4, 5
 SYMBOLS = [
     "dwf_create", "dwf_destroy", "dwf_set_option", "dwf_get_option", "dwf_set_stream", "dwf_set_gauge",
     "dwf_field_bytes", "dwf_pack", "dwf_unpack", "dwf_convert", "dwf_dhop", "dwf_meooe5d", "dwf_mooee",
-    "dwf_mooee_inv", "dwf_m", "dwf_mpc", "dwf_mdagm", "dwf_norm2", "dwf_cg", "dwf_multishift_cg", "dwf_chebyshev", "dwf_solve", "dwf_dhop_host",
+    "dwf_mooee_inv", "dwf_m", "dwf_mpc", "dwf_mdagm", "dwf_norm2", "dwf_cg", "dwf_multishift_cg", "dwf_chebyshev", "dwf_domain_project", "dwf_boundary_op", "dwf_solve", "dwf_dhop_host",
     "dwf_mdagm_host", "dwf_cg_host", "dwf_solve_host", "dwf_launch_count", "dwf_last_error", "dwf_version",
 ]
 
@@ -80,6 +80,8 @@ def load_library():
     lib.dwf_mdagm.argtypes = [vp, vp, vp, ci]
     lib.dwf_norm2.argtypes = [vp, vp, ci, ci, P(cd)]
     lib.dwf_cg.argtypes = [vp, vp, vp, cd, ci, ci, ci, P(CgInfo)]
+    lib.dwf_domain_project.argtypes = [vp, vp, vp, ci, ci]
+    lib.dwf_boundary_op.argtypes = [vp, vp, vp, ci, cd, ci, ci, P(CgInfo)]
     lib.dwf_chebyshev.argtypes = [vp, vp, vp, cd, cd, ci, ci]
     lib.dwf_multishift_cg.argtypes = [vp, vp, vp, P(cd), ci, cd, ci, P(CgInfo), P(cd)]
     lib.dwf_solve.argtypes = [vp, vp, vp, cd, ci, ci, P(CgInfo)]
@@ -260,6 +262,20 @@ class Dwf:
         st = self._chk(self.lib.dwf_cg(self._h, self._p(x), self._p(b), tol, max_iter, mode, int(use_guess),
                                        ctypes.byref(info)), allow=(ENOTCONV,))
         return x, info.as_dict(), st
+
+    def domain_project(self, inp, which, prec=F64, out=None):
+        """which = 0: P_Omega, 1: P_Omegabar, 2: boundary projector P_dbar; FULL native fields."""
+        out = self.new_native(prec, FULL) if out is None else out
+        self._chk(self.lib.dwf_domain_project(self._h, self._p(out), self._p(inp), int(which), prec))
+        return out
+
+    def boundary_op(self, phi, inverse, tol, max_iter, mode=CG_F64, out=None):
+        """R phi (inverse False, eq. 13) or R^-1 phi (inverse True, eq. 14); FULL fp64 native fields."""
+        out = self.new_native(F64, FULL) if out is None else out
+        info = CgInfo()
+        st = self._chk(self.lib.dwf_boundary_op(self._h, self._p(out), self._p(phi), int(bool(inverse)), tol, max_iter, mode,
+                                                ctypes.byref(info)), allow=(ENOTCONV,))
+        return out, info.as_dict(), st
 
     def chebyshev(self, inp, lo, hi, order, prec=F64, out=None):
         out = self.new_native(prec, ODD) if out is None else out

@@ -361,7 +361,10 @@ dwf_status dwf_destroy(dwf_ctx* c) {
         if (c->W64[p]) cudaFree(c->W64[p]);
         if (c->W32[p]) cudaFree(c->W32[p]);
         if (c->stage_dev[p]) cudaFree(c->stage_dev[p]);
+        if (c->W64u[p]) cudaFree(c->W64u[p]);
+        if (c->W32u[p]) cudaFree(c->W32u[p]);
     }
+    if (c->bnd_ws) cudaFree(c->bnd_ws);
     for (int i = 0; i < NWS; ++i) {
         if (c->ws64[i]) cudaFree(c->ws64[i]);
         if (c->ws32[i]) cudaFree(c->ws32[i]);
@@ -469,6 +472,14 @@ dwf_status dwf_set_gauge(dwf_ctx* c, const void* U) {
         if (c->W32[p] && c->wbytes32 != b32) { cudaFree(c->W32[p]); c->W32[p] = nullptr; }
         if (!c->W64[p] && cudaMalloc(&c->W64[p], b64) != cudaSuccess) { cudaGetLastError(); c->err = "cudaMalloc(gauge) failed"; return DWF_ENOMEM; }
         if (!c->W32[p] && cudaMalloc(&c->W32[p], b32) != cudaSuccess) { cudaGetLastError(); c->err = "cudaMalloc(gauge) failed"; return DWF_ENOMEM; }
+    }
+    const bool any_cut = c->cut[0] || c->cut[1] || c->cut[2] || c->cut[3];
+    select_links(c, false);
+    for (int p = 0; p < 2 && any_cut; ++p) {      // the same field without the cut, for the boundary operators (eqs. 8-14)
+        if (c->W64u[p] && c->wbytes64 != b64) { cudaFree(c->W64u[p]); c->W64u[p] = nullptr; }
+        if (c->W32u[p] && c->wbytes32 != b32) { cudaFree(c->W32u[p]); c->W32u[p] = nullptr; }
+        if (!c->W64u[p] && cudaMalloc(&c->W64u[p], b64) != cudaSuccess) { cudaGetLastError(); c->err = "cudaMalloc(gauge) failed"; return DWF_ENOMEM; }
+        if (!c->W32u[p] && cudaMalloc(&c->W32u[p], b32) != cudaSuccess) { cudaGetLastError(); c->err = "cudaMalloc(gauge) failed"; return DWF_ENOMEM; }
     }
     c->wbytes64 = b64;
     c->wbytes32 = b32;
@@ -745,6 +756,96 @@ dwf_status dwf_solve(dwf_ctx* c, void* psi, const void* eta, double tol, int max
     info->seconds = now_s() - t0;
     info->launches = (int)(c->launches - l0);
     return st;
+}
+
+// ---- domain / boundary projectors and the boundary operators R, R^-1 (eqs. 8-14)
+static dwf_status boundary_geometry_ok(dwf_ctx* c) {
+    bool any = false;
+    for (int mu = 0; mu < 4; ++mu)
+        if (c->cut[mu] > 0) {
+            any = true;
+            if ((c->g.L[mu] / c->cut[mu]) & 1) { c->err = "boundary operators need an even number of Dirichlet blocks in every cut direction"; return DWF_EINVAL; }
+        }
+    if (!any) { c->err = "boundary operators need a Dirichlet cut (dwf_create dirichlet_cut)"; return DWF_EINVAL; }
+    return DWF_OK;
+}
+
+dwf_status dwf_domain_project(dwf_ctx* c, void* out, const void* in, int which, dwf_prec prec) {
+    if (!c || !out || !in || which < 0 || which > 2) return DWF_EINVAL;
+    DWF_TRY(boundary_geometry_ok(c));
+    const size_t hb = half_bytes(c->g, prec);
+    for (int p = 0; p < 2; ++p) DWF_TRY(launch_domain_project(c, (char*)out + p * hb, (const char*)in + p * hb, p, which, prec));
+    return DWF_OK;
+}
+
+namespace {
+struct LinkGuard {      // the uncut link set is only ever visible inside one ABI call
+    dwf_ctx* c;
+    explicit LinkGuard(dwf_ctx* cc) : c(cc) {}
+    ~LinkGuard() { select_links(c, false); }
+};
+// out = P_to M_uncut P_from in  (the zero-padded boundary blocks of eq. 4: from = 0, to = 1 is D_dbar_hat; from = 1, to = 0 D_d_hat)
+dwf_status boundary_block(dwf_ctx* c, void* out, const void* in, void* tmp, int from, int to) {
+    DWF_TRY(dwf_domain_project(c, tmp, in, from, DWF_F64));
+    select_links(c, true);
+    DWF_TRY(m_apply(c, out, tmp, 0, DWF_F64));
+    select_links(c, false);
+    return dwf_domain_project(c, out, out, to, DWF_F64);
+}
+}  // namespace
+
+dwf_status dwf_boundary_op(dwf_ctx* c, void* out, const void* in, int inverse, double tol, int max_iter, dwf_cg_mode mode,
+                           dwf_cg_info* info) {
+    DWF_TRY(need_gauge(c));
+    dwf_cg_info local;
+    if (!info) info = &local;
+    memset(info, 0, sizeof(*info));
+    if (!out || !in || out == in || tol <= 0.0) { c->err = "boundary_op: bad arguments"; return DWF_EINVAL; }
+    DWF_TRY(boundary_geometry_ok(c));
+    const double t0 = now_s();
+    const long long l0 = c->launches;
+    const size_t fb = 2 * half_bytes(c->g, DWF_F64);
+    if (c->bnd_ws_bytes < 2 * fb) {
+        if (c->bnd_ws) cudaFree(c->bnd_ws);
+        c->bnd_ws = nullptr; c->bnd_ws_bytes = 0;
+        if (cudaMalloc(&c->bnd_ws, 2 * fb) != cudaSuccess) { cudaGetLastError(); c->err = "cudaMalloc(boundary workspace) failed"; return DWF_ENOMEM; }
+        c->bnd_ws_bytes = 2 * fb;
+    }
+    void* u = c->bnd_ws;
+    void* v = (char*)c->bnd_ws + fb;
+    LinkGuard guard(c);
+    dwf_cg_info si;
+    dwf_status st, worst = DWF_OK;
+    int iters = 0;
+    double rfull = 0.0;
+    DWF_TRY(boundary_block(c, u, in, v, 0, 1));                         // u = D_dbar_hat phi            (on Omegabar)
+    if (inverse) {
+        select_links(c, true);                                          // v = D^-1 u                    (eq. 14)
+        st = dwf_solve(c, v, u, tol, max_iter, mode, &si);
+        select_links(c, false);
+        if (st != DWF_OK && st != DWF_ENOTCONV) return st;
+        if (st != DWF_OK) worst = st;
+        iters += si.iters_total; rfull = si.resid_full;
+    } else {
+        st = dwf_solve(c, v, u, tol, max_iter, mode, &si);              // v = D_Ob^-1 u  (the cut operator is D_O + D_Ob)
+        if (st != DWF_OK && st != DWF_ENOTCONV) return st;
+        if (st != DWF_OK) worst = st;
+        iters += si.iters_total; rfull = si.resid_full;
+        DWF_TRY(boundary_block(c, u, v, out, 1, 0));                    // u = D_d_hat v                 (on Omega; out as scratch)
+        st = dwf_solve(c, v, u, tol, max_iter, mode, &si);              // v = D_O^-1 u                  (eq. 13)
+        if (st != DWF_OK && st != DWF_ENOTCONV) return st;
+        if (st != DWF_OK) worst = st;
+        iters += si.iters_total; rfull = std::fmax(rfull, si.resid_full);
+    }
+    DWF_TRY(dwf_domain_project(c, u, v, 2, DWF_F64));                   // P v
+    DWF_TRY(dwf_domain_project(c, out, in, 2, DWF_F64));                // P phi
+    DWF_TRY(launch_axpy(c, out, u, -1.0, DWF_F64, 2 * half_reals(c)));  // out = P phi - P v
+    cudaStreamSynchronize(c->stream);
+    info->iters_total = iters;
+    info->resid_full = rfull;
+    info->seconds = now_s() - t0;
+    info->launches = (int)(c->launches - l0);
+    return worst;
 }
 
 dwf_status dwf_dhop_host(dwf_ctx* c, void* out_host, const void* in_host, dwf_parity out_parity, int dagger, dwf_prec prec) {

@@ -49,16 +49,29 @@ dwf_status launch_gauge_prep(dwf_ctx* c, const double* Ucanon) {
     const Geom& g = c->g;
     const int ng = c->compress12 ? 12 : 18;
     const int block = 128, grid = (g.Vh * 8 + block - 1) / block;
-    for (int par = 0; par < 2; ++par) {
-        const int kg64 = (ng + 1) / 2 * 2, kg32 = (ng + 3) / 4 * 4;
-        gauge_prep_kernel<double><<<grid, block, 0, c->stream>>>(geom_prec(c, DWF_F64), Ucanon, (double*)c->W64[par], par, ng, kg64, 2,
-                                                                 c->cut[0], c->cut[1], c->cut[2], c->cut[3]);
-        gauge_prep_kernel<float><<<grid, block, 0, c->stream>>>(geom_prec(c, DWF_F32), Ucanon, (float*)c->W32[par], par, ng, kg32, 4,
-                                                                c->cut[0], c->cut[1], c->cut[2], c->cut[3]);
-        c->launches += 2;
+    const bool any_cut = c->cut[0] || c->cut[1] || c->cut[2] || c->cut[3];
+    for (int set = 0; set < (any_cut && c->W64u[0] ? 2 : 1); ++set) {      // 0: with the Dirichlet cut, 1: without
+        const int c0 = set ? 0 : c->cut[0], c1 = set ? 0 : c->cut[1], c2 = set ? 0 : c->cut[2], c3 = set ? 0 : c->cut[3];
+        for (int par = 0; par < 2; ++par) {
+            const int kg64 = (ng + 1) / 2 * 2, kg32 = (ng + 3) / 4 * 4;
+            gauge_prep_kernel<double><<<grid, block, 0, c->stream>>>(geom_prec(c, DWF_F64), Ucanon,
+                                                                     (double*)(set ? c->W64u[par] : c->W64[par]), par, ng, kg64, 2, c0, c1, c2, c3);
+            gauge_prep_kernel<float><<<grid, block, 0, c->stream>>>(geom_prec(c, DWF_F32), Ucanon,
+                                                                    (float*)(set ? c->W32u[par] : c->W32[par]), par, ng, kg32, 4, c0, c1, c2, c3);
+            c->launches += 2;
+        }
     }
     DWF_CUDA_CHECK(c, cudaGetLastError());
     return DWF_OK;
+}
+
+void select_links(dwf_ctx* c, bool uncut) {
+    if (c->links_uncut == uncut || !c->W64u[0]) return;
+    for (int p = 0; p < 2; ++p) {
+        void* t = c->W64[p]; c->W64[p] = c->W64u[p]; c->W64u[p] = t;
+        t = c->W32[p]; c->W32[p] = c->W32u[p]; c->W32u[p] = t;
+    }
+    c->links_uncut = uncut;
 }
 
 // ---- spinor layout conversion: canonical <-> native, native f32 <-> native f64 ------------------
@@ -88,6 +101,82 @@ __global__ void pack_kernel(Geom g, R* __restrict__ native, R* __restrict__ cano
         const size_t ni = native_real_index<R>(g, tile, lane, s, r);
         if (UNPACK) cp[r] = native[ni]; else native[ni] = cp[r];
     }
+}
+
+// ---- domain and boundary projectors (eqs. 1-2, 8 PAPER.md:42-50, 87-89) --------------
+// Omega = sites whose block indices floor(x_mu / B_mu), summed over the cut directions, are even.  The boundary projector
+// P_dbar acts on the sites of Omega that have a cut link ("mask and shift by one in each direction"): forward link cut
+// (x_mu mod B = B-1): the Omegabar neighbour reads (1 + gamma_mu) psi(x); backward link cut (x_mu mod B = 0): it reads
+// (1 - gamma_mu) psi(x).  Shamir, one cut face at the site: (1 +- gamma_mu)/2; otherwise (Moebius: A = b5 + c5 Q mixes s
+// and chirality; several faces): the identity on that site -- the smallest coordinate projector containing the minimal
+// one.  gamma matrices: chiral basis of reading C1.
+__device__ __forceinline__ void half_one_pm_gamma(int mu, double sg, const double (&v)[24], double (&o)[24]) {
+    // gamma_mu psi, spin index a = 0..3, complex (re, im) per colour: rows listed as (source spin, factor) with factor in {1,-1,i,-i}
+    // gx: (3,i)(2,i)(1,-i)(0,-i)  gy: (3,-1)(2,1)(1,1)(0,-1)  gz: (2,i)(3,-i)(0,-i)(1,i)  gt: (2,1)(3,1)(0,1)(1,1)
+    const int src[4][4] = {{3, 2, 1, 0}, {3, 2, 1, 0}, {2, 3, 0, 1}, {2, 3, 0, 1}};
+    const int fre[4][4] = {{0, 0, 0, 0}, {-1, 1, 1, -1}, {0, 0, 0, 0}, {1, 1, 1, 1}};      // real part of the factor
+    const int fim[4][4] = {{1, 1, -1, -1}, {0, 0, 0, 0}, {1, -1, -1, 1}, {0, 0, 0, 0}};    // imaginary part of the factor
+    for (int a = 0; a < 4; ++a) {
+        const int b = src[mu][a];
+        const double fr = fre[mu][a], fi = fim[mu][a];
+        for (int cc = 0; cc < 3; ++cc) {
+            const double xr = v[(b * 3 + cc) * 2], xi = v[(b * 3 + cc) * 2 + 1];
+            const double gr = fr * xr - fi * xi, gi = fr * xi + fi * xr;
+            o[(a * 3 + cc) * 2] = 0.5 * (v[(a * 3 + cc) * 2] + sg * gr);
+            o[(a * 3 + cc) * 2 + 1] = 0.5 * (v[(a * 3 + cc) * 2 + 1] + sg * gi);
+        }
+    }
+}
+
+template <typename R>
+__global__ void domain_project_kernel(Geom g, R* __restrict__ out, const R* __restrict__ in, int parity, int which, int cut0,
+                                      int cut1, int cut2, int cut3, int shamir) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= (long long)g.Vh * g.Ls) return;
+    const int s = (int)(gid % g.Ls);
+    const int site = (int)(gid / g.Ls);
+    const int tile = site / g.TS, lane = site - tile * g.TS;
+    const int cut[4] = {cut0, cut1, cut2, cut3};
+    const Coord c = site_coords(g, tile, lane, parity);
+    int blk = 0, nface = 0, fmu = 0;
+    double fsg = 0.0;
+    for (int mu = 0; mu < 4; ++mu) {
+        const int B = cut[mu];
+        if (B <= 0) continue;
+        blk += c.x[mu] / B;
+        const int r = c.x[mu] % B;
+        if (r == B - 1) { ++nface; fmu = mu; fsg = 1.0; }
+        if (r == 0) { ++nface; fmu = mu; fsg = -1.0; }
+    }
+    const bool omega = (blk & 1) == 0;
+    double v[24], o[24];
+    for (int r = 0; r < 24; ++r) v[r] = (double)in[native_real_index<R>(g, tile, lane, s, r)];
+    bool keep;
+    if (which == 0) keep = omega;
+    else if (which == 1) keep = !omega;
+    else keep = omega && nface > 0;
+    if (keep && which == 2 && shamir && nface == 1) {
+        half_one_pm_gamma(fmu, fsg, v, o);
+    } else {
+        for (int r = 0; r < 24; ++r) o[r] = keep ? v[r] : 0.0;
+    }
+    for (int r = 0; r < 24; ++r) out[native_real_index<R>(g, tile, lane, s, r)] = (R)o[r];
+}
+
+dwf_status launch_domain_project(dwf_ctx* c, void* out, const void* in, int parity, int which, int prec) {
+    const Geom g = geom_prec(c, prec);
+    const long long n = (long long)g.Vh * g.Ls;
+    const int block = 128, grid = (int)((n + block - 1) / block);
+    const int shamir = (c->c5 == 0.0) ? 1 : 0;
+    if (prec == DWF_F64)
+        domain_project_kernel<double><<<grid, block, 0, c->stream>>>(g, (double*)out, (const double*)in, parity, which, c->cut[0],
+                                                                     c->cut[1], c->cut[2], c->cut[3], shamir);
+    else
+        domain_project_kernel<float><<<grid, block, 0, c->stream>>>(g, (float*)out, (const float*)in, parity, which, c->cut[0],
+                                                                    c->cut[1], c->cut[2], c->cut[3], shamir);
+    c->launches++;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    return DWF_OK;
 }
 
 dwf_status launch_pack(dwf_ctx* c, void* native, const void* canon, int prec, int parity, bool unpack) {

@@ -80,6 +80,13 @@ struct dwf_ctx {
     void* W64[2] = {nullptr, nullptr};
     void* W32[2] = {nullptr, nullptr};
     size_t wbytes64 = 0, wbytes32 = 0;
+    // second link set WITHOUT the Dirichlet cut (built when a cut is configured): the boundary operators of eqs. 8-14 need
+    // D and D_Omega + D_Omegabar on the same gauge field.  select_links() swaps it with W64 / W32.
+    void* W64u[2] = {nullptr, nullptr};
+    void* W32u[2] = {nullptr, nullptr};
+    bool links_uncut = false;
+    void* bnd_ws = nullptr;      // boundary operators: two FULL fp64 fields
+    size_t bnd_ws_bytes = 0;
     dwf::Table5 tab[dwf::OP5_COUNT];
     dwf::DevTables dtab;
     // workspace (allocated lazily, sized for half fields)
@@ -133,6 +140,9 @@ dwf_status launch_dhop(dwf_ctx* c, void* out, const void* in, int out_parity, in
 dwf_status launch_op5(dwf_ctx* c, void* out, const void* x, int op1, const void* y, int op2, double yscale,
                       int prec, int norm_slot);
 dwf_status launch_gauge_prep(dwf_ctx* c, const double* Ucanon);
+void select_links(dwf_ctx* c, bool uncut);   // which link set the operators see (must be back on `cut` when an ABI call returns)
+// out = P in on one half field of `parity`: which = 0 P_Omega, 1 P_Omegabar, 2 the boundary projector P_dbar (fp64 or fp32)
+dwf_status launch_domain_project(dwf_ctx* c, void* out, const void* in, int parity, int which, int prec);
 dwf_status launch_pack(dwf_ctx* c, void* native, const void* canon, int prec, int parity, bool unpack);
 dwf_status launch_convert(dwf_ctx* c, void* dst, int dprec, const void* src, int sprec, size_t nhalf_fields);
 // BLAS-1 on native half fields; scalar slots index c->scalars
