@@ -56,6 +56,17 @@ def run(cfg, U, b_np, with_sweeps=True, max_iter=50000, extras=False):
         rep[name] = {"tol": cfg.tol, "status": int(st), "iters": info["iters_total"], "restarts": info["restarts"],
                      "resid_true": info["resid_true"], "seconds": info["seconds"], "launches": info["launches"]}
         del x
+    if extras and any(cfg.cut) and all(c == 0 or (d // c) % 2 == 0 for d, c in zip(cfg.dims, cfg.cut)):
+        # the boundary operators R^-1 (one uncut solve) and R (two Dirichlet solves), eqs. 13-14
+        phi = g.new_native(A.F64, A.FULL).normal_()
+        p = g.domain_project(phi, 2)
+        rinv, i1, st1 = g.boundary_op(phi, True, cfg.tol, max_iter, A.CG_MIXED)
+        rr, i2, st2 = g.boundary_op(rinv, False, cfg.tol, max_iter, A.CG_MIXED)
+        rep["boundary"] = {"Rinv": {"status": int(st1), "iters": i1["iters_total"], "seconds": i1["seconds"]},
+                           "R": {"status": int(st2), "iters": i2["iters_total"], "seconds": i2["seconds"]},
+                           "R_Rinv_minus_P_rel": float(torch.linalg.norm(rr - p) / torch.linalg.norm(p)),
+                           "boundary_fraction": float((p != 0).sum() / p.numel())}
+        del phi, p, rinv, rr
     if extras:
         # SURVEY 8f NEXT-2 / NEXT-4 at full size: four shifts in one Krylov space; a 16th-order Chebyshev filter
         shifts = [0.0, 0.01, 0.1, 1.0]
