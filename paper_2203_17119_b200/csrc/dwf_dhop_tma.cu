@@ -1,17 +1,17 @@
-// Dhop, warp-specialised TMA kernel for 4x4x4x4 tiles (the fast path on sm_100a).
+// Dhop, warp-specialised TMA kernel for 4x4x4x4 tiles (the fast path on sm_100a; DESIGN.md section 5.1).
 //
-// Persistent CTAs walk the tiles in an L2-friendly sweep order.  Per CTA:
+// Persistent CTAs take tiles from a global in-order queue over an L2-friendly sweep order.  Per CTA:
 //   * warp group 0 is the PRODUCER (one warp active, registers shrunk with setmaxnreg): for every
 //     (tile, s) it fills one stage of an NST-deep shared-memory ring with the s-slice working set of
 //     the tile -- 12 regions of [K][32 slots] 16-byte vectors:
 //        regions 0-3   the tile's own four t-slabs           (TMA, 512-byte rows)
 //        regions 4,5   +t / -t faces of the neighbour tiles  (TMA, 512-byte rows)
 //        regions 6,7   +z / -z faces                         (TMA, 128-byte rows)
-//        regions 8,9   +y / -y faces                         (TMA, 32-byte rows)
+//        regions 8,9   +y / -y faces                         (fp32: TMA, 32-byte rows; fp64: cp.async gather)
 //        regions 10,11 +x / -x faces                         (cp.async gather: the checkerboard makes the x
 //                                                             face a row-parity pattern no box can describe)
-//     ten cp.async.bulk.tensor boxes + 2K cp.async per lane, all completing on the stage's `full`
-//     mbarrier; the next tile's links are prefetched into L2 with one bulk prefetch;
+//     all completing on the stage's `full` mbarrier; the next tile's links are prefetched into L2 with one bulk
+//     prefetch issued with the tile's last slice;
 //   * the other warp groups are CONSUMERS: each thread keeps its links in registers for the whole s
 //     loop (third row rebuilt once per tile, antiperiodic sign folded in), waits on `full`, reads its
 //     neighbours with 128-bit LDS at a uniform 512-byte k pitch, spin-projects, multiplies,
@@ -19,7 +19,9 @@
 //     coalesced with a streaming hint.  No block-wide barrier inside the loop: warps drift apart and
 //     keep the FP and shared-memory pipes busy at the same time.
 // fp32: one thread per site (8 links in registers), 2 CTAs/SM.  fp64: two lanes (l, l^16) per site (forward legs
-// on one, backward legs on the other), partial sums exchanged by warp shuffles, 1 CTA/SM.
+// on one, backward legs on the other), partial sums exchanged by warp shuffles, 1 CTA/SM; its fields use the
+// XOR-rotated lane order of dwf_layout.cuh and conflict-free face slots (build_tma_tables_swz).
+// EPI = 1 adds the last step of Mpc as an epilogue: out_s = Mee xin_s + scale (Dhop in)_s and its |.|^2.
 #include <cuda.h>
 
 #include <algorithm>
