@@ -246,7 +246,7 @@ def test_multishift_cg_matches_oracle(case):
     oracle's multishift CG, shared iteration count within +-2, true residuals recomputed by the oracle."""
     from oracle.dwf_oracle import multishift_cg
     g, A = case.gpu, case.api
-    if int(np.prod(case.dims)) * case.Ls > 30000:
+    if int(np.prod(case.dims)) * case.Ls > 13000:
         pytest.skip("the oracle's multishift CG takes minutes on this lattice; the smaller ones cover every code path")
     shifts = [0.0, 0.02, 0.4, 3.0]
     tol = 1e-10
