@@ -34,11 +34,11 @@ class Case:
     run on the fp32-rounded gauge and source, SURVEY §8(c) 'other silent points' (iii))."""
 
     def __init__(self, api, dims, Ls, par, eps=0.4, cut=(0, 0, 0, 0), apbc=True, seed=7, compress12=1, tiles=None, fuse=1,
-                 fused=None):
+                 fused=None, kernel=0):
         from oracle.dwf_oracle import Oracle
         self.api, self.dims, self.Ls = api, tuple(dims), Ls
         self.U = inputs.gauge_weak(dims, eps, seed)
-        opts = dict(antiperiodic_t=int(apbc), compress12=compress12, fuse=fuse)
+        opts = dict(antiperiodic_t=int(apbc), compress12=compress12, fuse=fuse, dhop_kernel=kernel)
         self.fused = fused
         if tiles:
             opts.update({f"tile_{k}": v for k, v in zip("xyzt", tiles)})
@@ -94,6 +94,10 @@ CASES = {
     "fused12_shamir": dict(dims=(4, 8, 8, 4), Ls=12, par=SHAM, eps=0.5, apbc=False, fused=True),
     "unfused12": dict(dims=(8, 8, 4, 8), Ls=12, par=MOEB, eps=0.5, fuse=0, fused=False),
     "c1_unfused": dict(dims=(4, 4, 4, 4), Ls=8, par=SHAM, eps=0.2, fuse=0, fused=False),
+    # 4^4 tiles (fp64 fields in the XOR-rotated lane order) through the other two Dhop kernels: the cp.async tile kernel
+    # (dhop_kernel = 2) and the shape-generic kernel (dhop_kernel = 1); they never run the fused epilogue
+    "pipe_kernel_on_4x4x4x4": dict(dims=(8, 4, 8, 4), Ls=8, par=MOEB, eps=0.5, kernel=2, fuse=0, fused=False),
+    "generic_kernel_on_4x4x4x4": dict(dims=(4, 8, 4, 8), Ls=6, par=MOEB, eps=0.5, kernel=1, fuse=0, fused=False),
 }
 
 
