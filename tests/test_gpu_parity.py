@@ -283,3 +283,24 @@ def test_chebyshev_filter_matches_oracle(case, prec):
         assert rel(got, chebyshev(orc, o, lo, hi, order)) < (1e-11 if prec == "f64" else 2e-5), order
     with pytest.raises(A.DwfError):
         g.chebyshev(nat, 1.0, 1.0, 3, P)
+
+
+def test_cg_initial_guess_and_mixed_full_solve(case):
+    """dwf_cg with use_guess (reading C8: r = b - A x_0 first) and dwf_solve in mixed precision (C6 + C9)."""
+    g, A = case.gpu, case.api
+    b = g.pack(case.odd, A.F64, A.ODD)
+    x0, info0, st = g.cg(b, 1e-5, 5000, A.CG_F64)
+    assert st == A.OK
+    xcold, cold, st = g.cg(b, 1e-10, 5000, A.CG_F64)
+    x1, warm, st = g.cg(b, 1e-10, 5000, A.CG_F64, x=x0.clone(), use_guess=True)
+    assert st == A.OK and warm["resid_true"] <= 1e-10
+    assert warm["iters_total"] < cold["iters_total"]
+    xs = g.unpack(x1, A.F64, A.ODD)
+    assert np.sqrt(case.orc.norm2(case.odd - case.orc.mdagm(xs)) / case.orc.norm2(case.odd)) <= 1e-10 * (1 + 1e-6)
+    x2, again, st = g.cg(b, 1e-9, 5000, A.CG_F64, x=xcold.clone(), use_guess=True)       # already converged: nothing to do
+    assert st == A.OK and again["iters_total"] == 0
+    psi, info, st = g.solve(case.full_native("f64"), 1e-10, 20000, A.CG_MIXED)
+    assert st == A.OK and info["restarts"] >= 1
+    got = case.unpack_full(psi, "f64")
+    res = np.sqrt(case.orc.norm2(case.full - case.orc.M(got)) / case.orc.norm2(case.full))
+    assert res < 1e-7 and abs(info["resid_full"] - res) <= 1e-3 * res + 1e-13
