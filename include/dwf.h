@@ -93,7 +93,10 @@ dwf_status dwf_set_stream(dwf_ctx* ctx, void* cuda_stream);
 
 /* Copies a canonical fp64 gauge field (device pointer, V4*4*18 doubles) into the context: applies the
  * Dirichlet cut, builds the 8-legs-per-site native copies (forward U_mu(x), backward U_mu(x-mu)^dag) in
- * fp64 and fp32 (round to nearest) for both parities, optionally 2-row compressed. */
+ * fp64 and fp32 (round to nearest) for both parities, optionally 2-row compressed.  When a Dirichlet cut is configured
+ * the same copies are also kept WITHOUT the cut (used only inside dwf_boundary_op; every other operator sees the cut
+ * links).  The native layout is opaque and precision-specific (fp64 and fp32 fields order the sites of a
+ * tile differently): move data between precisions with dwf_convert, never by casting a native buffer. */
 dwf_status dwf_set_gauge(dwf_ctx* ctx, const void* U_dev_canonical_f64);
 
 /* Bytes of a native field of the given precision and parity (DWF_FULL = 2 x half). */
