@@ -168,18 +168,6 @@ void ORC(orc_dhop)(const orc_params* p, const real* U, const real* in_, real* ou
     }
 }
 
-/* The same per-site loop for a LIST of output sites (full-lattice lex indices, each of parity
- * out_parity when out_parity != 2): out[i] = Dhop in at site lex_list[i], [i][s][spin][colour].
- * Lets the tests check sampled outputs at sizes where a full oracle pass is slow.              */
-void ORC(orc_dhop_sites)(const orc_params* p, const real* U, const real* in_, real* out_, int out_parity,
-                         int dagger, long nsites, const long* lex_list) {
-    const cplx* in = (const cplx*)in_;
-    cplx* out = (cplx*)out_;
-    const cplx* Uc = (const cplx*)U;
-#pragma omp parallel for schedule(static)
-    for (long i = 0; i < nsites; ++i) dhop_site(p, Uc, in, out, lex_list[i], i, out_parity, dagger);
-}
-
 /* ---- C4: s-hop Q and its adjoint ---------------------------------------
  * (Q psi)_s  = P_- psi_{s+1} + P_+ psi_{s-1},  psi_{Ls} = -mf psi_0,
  *                                              psi_{-1} = -mf psi_{Ls-1}

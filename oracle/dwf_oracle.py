@@ -95,16 +95,6 @@ class Oracle:
                              int(out_parity), int(bool(dagger)))
         return out
 
-    def dhop_sites(self, psi, lex_list, out_parity=2, dagger=False):
-        """Dhop at the listed output sites only (full-lattice lex indices): [i, s, spin, colour]."""
-        psi = self._c(psi)
-        assert psi.shape == (self.full_shape() if out_parity == 2 else self.half_shape())
-        lex = np.ascontiguousarray(lex_list, dtype=np.int64)
-        out = np.empty((lex.size, self.Ls, 4, 3), dtype=self.cdtype)
-        self._fn("orc_dhop_sites")(ctypes.byref(self.p), self._ptr(self.U), self._ptr(psi), self._ptr(out),
-                                   int(out_parity), int(bool(dagger)), ctypes.c_long(lex.size), self._ptr(lex))
-        return out
-
     def _site_local(self, name, psi, dagger):
         psi = self._c(psi)
         n4 = psi.size // (self.Ls * 12)
@@ -296,7 +286,7 @@ def cg_mixed(orc64: Oracle, orc32: Oracle, b, tol, max_iter, inner_tol=1e-4, max
     x = np.zeros_like(b) if x0 is None else np.array(x0, dtype=np.complex128, copy=True)
     bnorm2 = orc64.norm2(b)
     iters_inner, restarts = 0, 0
-    per_restart = []
+    per_restart, deltas = [], []
     while True:
         r = b - orc64.mdagm(x)
         rn2 = orc64.norm2(r)
@@ -307,10 +297,11 @@ def cg_mixed(orc64: Oracle, orc32: Oracle, b, tol, max_iter, inner_tol=1e-4, max
         e, info = cg(orc32, r.astype(np.complex64), delta, max_iter - iters_inner, restart_on_true=False)
         iters_inner += info["iters"]
         per_restart.append(info["iters"])
+        deltas.append(float(delta))
         x += e.astype(np.complex128)
         restarts += 1
     return x, dict(iters=iters_inner, iters_inner=iters_inner, restarts=restarts, resid_true=float(resid_true),
-                   per_restart=per_restart, converged=bool(resid_true <= tol))
+                   per_restart=per_restart, deltas=deltas, converged=bool(resid_true <= tol))
 
 
 # ---------------------------------------------------------------------------

@@ -120,3 +120,48 @@ def domain_index(dims, Ls, mu, B):
 def Gamma5R5(V, Ls):
     R5 = np.eye(Ls)[::-1]
     return np.kron(np.eye(V), np.kron(R5, np.kron(G5, np.eye(3))))
+
+
+def domains_from_matrices(M, Mcut, dims, Ls):
+    """Omega / Omegabar read off the dense operators alone (eqs. 1-4): the sites fall into the connected
+    components of the Dirichlet-cut operator Mcut (its blocks), and every link that the cut removed (a non-zero site block
+    of M - Mcut) must join the two domains, which 2-colours the blocks; the block holding the origin is in Omega.
+    Returns (om, ob) index arrays into the 5-D dense vector, or raises if no such colouring exists."""
+    V = int(np.prod(dims))
+    n = Ls * 12
+
+    def site_adj(A):
+        return np.abs(A.reshape(V, n, V, n)).max(axis=(1, 3)) > 0
+
+    conn, removed = site_adj(Mcut), site_adj(M - Mcut)
+    comp = -np.ones(V, dtype=int)
+    nc = 0
+    for s0 in range(V):
+        if comp[s0] >= 0:
+            continue
+        stack = [s0]
+        comp[s0] = nc
+        while stack:
+            a = stack.pop()
+            for b in np.nonzero(conn[a])[0]:
+                if comp[b] < 0:
+                    comp[b] = nc
+                    stack.append(b)
+        nc += 1
+    colour = -np.ones(nc, dtype=int)
+    colour[comp[0]] = 0
+    changed = True
+    while changed:
+        changed = False
+        for a, b in zip(*np.nonzero(removed)):
+            ca, cb = comp[a], comp[b]
+            if colour[ca] >= 0 and colour[cb] < 0:
+                colour[cb] = 1 - colour[ca]
+                changed = True
+            elif colour[ca] >= 0 and colour[cb] >= 0 and colour[ca] == colour[cb]:
+                raise ValueError("a cut link joins two blocks of the same domain")
+    assert (colour >= 0).all()
+    site_dom = colour[comp]
+    om = np.concatenate([np.arange(s * n, (s + 1) * n) for s in range(V) if site_dom[s] == 0])
+    ob = np.concatenate([np.arange(s * n, (s + 1) * n) for s in range(V) if site_dom[s] == 1])
+    return om, ob, nc

@@ -66,6 +66,34 @@ def test_gauge_is_su3_and_plaquette_fingerprint():
     assert np.allclose(Uh @ np.conj(np.swapaxes(Uh, -1, -2)), np.eye(3), atol=1e-13)
 
 
+def test_haar_ape_generator_of_c5():
+    """The c5 gauge recipe (Haar SU(3) + 4 APE passes, alpha = 0.5) against what is known without running it:
+    Haar links have <Re tr P>/3 = 0 and <|U_ij|^2> = 1/3; a pure-gauge field is a fixed point of the smearing (every staple
+    equals the link); each pass raises the plaquette.  The value after 4 passes, 0.60 (0.597 on 8^4, 0.604 on the c5
+    lattice), is the recipe's fingerprint, kept to +-1 % so a changed alpha, staple or pass count shows."""
+    dims = (8, 8, 8, 8)
+    cfg = inputs.CONFIGS["c5"]
+    U0 = inputs.gauge_haar(dims, cfg.gauge_seed)
+    assert np.allclose(U0 @ np.conj(np.swapaxes(U0, -1, -2)), np.eye(3), atol=1e-13)
+    assert np.allclose(np.linalg.det(U0), 1.0, atol=1e-13)
+    nplaq = 6 * int(np.prod(dims))
+    assert abs(inputs.plaquette(U0)) < 4.0 / np.sqrt(nplaq)          # variance of Re tr P / 3 for Haar links is 1/18 < 1
+    assert abs(np.mean(np.abs(U0) ** 2) - 1.0 / 3.0) < 1e-12
+    plaq = [inputs.plaquette(U0)]
+    Us = U0
+    for _ in range(4):
+        Us = inputs.ape_smear(Us, 0.5, 1)
+        plaq.append(inputs.plaquette(Us))
+    assert all(b > a for a, b in zip(plaq, plaq[1:]))
+    assert np.allclose(Us @ np.conj(np.swapaxes(Us, -1, -2)), np.eye(3), atol=1e-13)
+    assert abs(plaq[-1] - 0.60) < 0.006
+    assert np.array_equal(inputs.make_gauge(inputs.small_variant(cfg, dims)), Us)          # make_gauge(c5) is this recipe
+    g = inputs.gauge_haar((4, 4, 4, 4), 7)[..., 0, :, :]
+    Ug = np.stack([g @ np.conj(np.swapaxes(np.roll(g, -1, axis=3 - mu), -1, -2)) for mu in range(4)], axis=4)
+    assert abs(inputs.plaquette(Ug) - 1.0) < 1e-14
+    assert np.abs(inputs.ape_smear(Ug, 0.5, 2) - Ug).max() < 1e-14
+
+
 def test_split_merge_roundtrip():
     f = inputs.source_full(DIMS, LS, 5)
     e, o = inputs.split_parity(f, DIMS)
@@ -386,6 +414,64 @@ def test_mixed_cg(U, psi, oracle_built):
     assert rel(x, x64) < 1e-8
     # the fp32 oracle is the fp64 oracle in lower precision
     assert rel(o32.mpc(b.astype(np.complex64)).astype(np.complex128), o64.mpc(b)) < 1e-6
+
+
+def test_mixed_cg_restarts_and_deltas_vs_dense_defect_correction(U, psi, oracle_built):
+    """Reading C9 pinned through its constants, not only its answer: the same defect correction written out around numpy's
+    dense matrices (fp64 outer residual with the dense Mpc^dag Mpc, inner CG with the complex64 copy of the dense Mpc and
+    fp64 reductions, delta = max(inner_tol, tol |b| / |r|)) must give the oracle's restart count, its delta sequence and
+    its inner iteration counts.  A wrong delta rule, a missing restart or an inner solve that does not start from e = 0
+    changes these numbers even when the final answer still converges."""
+    par = MOEB
+    o64, o32 = make(par, U), make(par, U, prec="f32")
+    M = dr.dwf_matrix(U, DIMS, LS, par["M5"], par["mf"], par["b5"], par["c5"])
+    ev, od = dr.parity_index(DIMS, LS)
+    Mpc = M[np.ix_(od, od)] - M[np.ix_(od, ev)] @ np.linalg.solve(M[np.ix_(ev, ev)], M[np.ix_(ev, od)])
+    Mpc32 = Mpc.astype(np.complex64)
+    Mpc32h = np.ascontiguousarray(Mpc32.conj().T)
+    _, b = split(psi, DIMS)
+    bv = b.reshape(-1)
+    for tol, inner_tol in ((1e-10, 1e-4), (1e-9, 1e-2), (1e-12, 1e-5)):
+        n2 = lambda v: float(np.sum(np.abs(v.astype(np.complex128)) ** 2))
+        x = np.zeros_like(bv)
+        bn2 = n2(bv)
+        deltas, inner, restarts = [], [], 0
+        while True:
+            r = bv - Mpc.conj().T @ (Mpc @ x)
+            rn2 = n2(r)
+            if np.sqrt(rn2 / bn2) <= tol or restarts >= 20:
+                break
+            delta = max(inner_tol, tol * np.sqrt(bn2 / rn2))
+            rf = r.astype(np.complex64)
+            e = np.zeros_like(rf)
+            p = rf.copy()
+            c = n2(rf)
+            target = delta * delta * c
+            k = 0
+            while c > target:
+                q = Mpc32 @ p
+                alpha = np.float32(c / n2(q))
+                e += alpha * p
+                rf -= alpha * (Mpc32h @ q)
+                cn = n2(rf)
+                k += 1
+                if cn <= target:
+                    break
+                p = rf + np.float32(cn / c) * p
+                c = cn
+            x = x + e.astype(np.complex128)
+            deltas.append(delta)
+            inner.append(k)
+            restarts += 1
+        xo, info = cg_mixed(o64, o32, b, tol, 5000, inner_tol=inner_tol)
+        assert info["converged"] and info["restarts"] == restarts and restarts >= 2, (info, restarts)
+        assert len(info["deltas"]) == restarts
+        # a delta above inner_tol is tol |b| / |r| with |r| at the fp32 rounding floor of the previous inner solve, which
+        # depends on the rounding order of the two operator implementations: same value within a factor 1.5
+        for dg, dw in zip(info["deltas"], deltas):
+            assert dg == dw if dw == inner_tol else (dg > inner_tol and 1 / 1.5 < dg / dw < 1.5), (info["deltas"], deltas)
+        assert all(abs(a - b_) <= 1 for a, b_ in zip(info["per_restart"], inner)), (info["per_restart"], inner)
+        assert rel(xo.reshape(-1), x) < 1e-7
 
 
 def test_zero_rhs_and_zero_links(oracle_built):
