@@ -77,7 +77,7 @@ def pair(request, oracle_built):
     if request.param == "c2":
         cfg = inputs.CONFIGS["c2"]
         p = Pair(api, cfg.dims, cfg.Ls, dict(M5=cfg.M5, mf=cfg.mf, b5=cfg.b5, c5=cfg.c5), cfg.eps, cfg.gauge_seed, cfg.cut[3])
-        p.with_oracle = False
+        p.with_oracle = True
     else:
         p = Pair(api, (8, 8, 8, 16), 8, MOEB, 0.3, 11, 8)
         p.with_oracle = True
@@ -102,7 +102,8 @@ def test_cut_operator_is_block_diagonal_and_restricts_D(pair):
         par = pair.par
         orc = Oracle(pair.dims, pair.Ls, par["M5"], par["mf"], par["b5"], par["c5"], antiperiodic_t=True,
                      cut=(0, 0, 0, 8)).set_gauge(pair.U)
-        assert rel(Mc, orc.M(v_om)) < 1e-12
+        want = orc.M(v_om)
+        assert rel(Mc, want) < 1e-12 and float(np.abs(Mc - want).max() / np.abs(want).max()) < 1e-12
 
 
 def test_eq5_schur_factorisation_on_a_random_vector(pair):
@@ -126,3 +127,31 @@ def test_eq5_schur_factorisation_on_a_random_vector(pair):
         par = pair.par
         orc = Oracle(pair.dims, pair.Ls, par["M5"], par["mf"], par["b5"], par["c5"], antiperiodic_t=True).set_gauge(pair.U)
         assert rel(z, orc.M(v)) < 1e-8
+
+
+@pytest.mark.slow
+def test_c2_cg_to_completion_matches_oracle(oracle_built):
+    """"oracle CG run to completion" -- BASELINE configs[1] at full size (16^4 x 16 Moebius, cut B_t = 8,
+    tol 1e-10): Mpc^dag Mpc of the cut operator whole-field against the oracle, then the red-black CG on both sides with the
+    iteration count within +-2 (north_star) and the oracle recomputing the true residual of the GPU solution."""
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    from paper_2203_17119_b200 import api as A
+    from oracle.dwf_oracle import Oracle, cg
+    cfg = inputs.CONFIGS["c2"]
+    U = inputs.make_gauge(cfg)
+    g = A.from_config(cfg, device="cuda:0")
+    g.set_gauge(U)
+    orc = Oracle(cfg.dims, cfg.Ls, cfg.M5, cfg.mf, cfg.b5, cfg.c5, antiperiodic_t=cfg.antiperiodic_t, cut=cfg.cut).set_gauge(U)
+    odd = inputs.source_half(cfg.dims, cfg.Ls, cfg.source_seed, parity=1)
+    nat = g.pack(odd, A.F64, A.ODD)
+    got, want = g.unpack(g.mdagm(nat, A.F64), A.F64, A.ODD), orc.mdagm(odd)
+    assert rel(got, want) < 2e-12 and float(np.abs(got - want).max() / np.abs(want).max()) < 2e-12
+    x_ref, info_ref = cg(orc, odd, cfg.tol, 5000)
+    x, info, st = g.cg(nat, cfg.tol, 5000, A.CG_F64)
+    assert st == A.OK and info_ref["converged"] and info["resid_true"] <= cfg.tol
+    assert abs(info["iters_total"] - info_ref["iters"]) <= 2, (info, info_ref)
+    xs = g.unpack(x, A.F64, A.ODD)
+    assert np.sqrt(orc.norm2(odd - orc.mdagm(xs)) / orc.norm2(odd)) <= cfg.tol * (1 + 1e-6)
+    assert rel(xs, x_ref) < 1e-5
+    g.close()

@@ -250,10 +250,11 @@ def test_multishift_cg_matches_oracle(case):
     oracle's multishift CG, shared iteration count within +-2, true residuals recomputed by the oracle."""
     from oracle.dwf_oracle import multishift_cg
     g, A = case.gpu, case.api
-    if int(np.prod(case.dims)) * case.Ls > 13000 or case.Ls == 5:
-        pytest.skip("the oracle's multishift CG takes minutes on this lattice; the smaller ones cover every code path")
-    shifts = [0.0, 0.02, 0.4, 3.0]
-    tol = 1e-10
+    # the oracle's multishift CG takes minutes to 1e-10 with four shifts on the larger lattices (every Ls = 12 / 16 one and the
+    # generic-Ls one): two shifts to 1e-6 there -- same kernels, same recurrences, fewer iterations
+    slow = int(np.prod(case.dims)) * case.Ls > 13000 or case.Ls == 5
+    shifts = [0.0, 0.4] if slow else [0.0, 0.02, 0.4, 3.0]
+    tol = 1e-6 if slow else 1e-10
     xs_ref, info_ref = multishift_cg(case.orc, case.odd, shifts, tol, 5000)
     xs, info, res, st = g.multishift_cg(g.pack(case.odd, A.F64, A.ODD), shifts, tol, 5000)
     assert st == A.OK and info_ref["converged"]
@@ -261,7 +262,7 @@ def test_multishift_cg_matches_oracle(case):
     bn2 = case.orc.norm2(case.odd)
     for x, xr, sg, rt in zip(xs, xs_ref, shifts, res):
         got = g.unpack(x, A.F64, A.ODD)
-        assert rel(got, xr) < 1e-6
+        assert rel(got, xr) < (1e-3 if slow else 1e-6)
         true_res = np.sqrt(case.orc.norm2(case.odd - case.orc.mdagm(got) - sg * got) / bn2)
         assert true_res <= 2 * tol and abs(true_res - rt) <= 1e-3 * true_res + 1e-14
     with pytest.raises(A.DwfError):
