@@ -13,8 +13,9 @@ dwf_cg_host with pinned HOST buffers (H2D/D2H copies and layout packing inside t
 `roofline` is the dominant kernel (half-volume fp64 Dhop) timed per launch by CUDA events on the launching
 stream inside the timed steps.  Extra keys report the Dhop / Mpc^dag Mpc sweeps and CG time-to-solution.
 
-N > 1 (torchrun): the path shards by independent Dirichlet subdomains, one per rank, no
-data-path collective; timing is the max over ranks ("scaling": "weak").
+N > 1 (torchrun): replicas only -- every rank runs the same step on its own seeded
+copy of the workload lattice (the paper's situation: one Dirichlet subdomain per GPU, solved with no communication,
+PAPER.md:123); there is no data-path collective, timing is the max over ranks ("scaling": "weak").
 --impl reference: the CPU oracle (oracle/), as it stands, on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -105,38 +106,106 @@ def make_inputs(cfg, rank: int):
 
 
 # ------------------------------------------------------------------------------------------- reference arm
-def oracle_segment(sample_dims, cfg, iters, steps, warmup):
-    """The oracle's CG (oracle/dwf_oracle.py cg, as it stands) for `iters` iterations on a sample lattice."""
-    from oracle.dwf_oracle import Oracle, cg
-    from paper_2203_17119_b200 import inputs
-    U = inputs.gauge_weak(sample_dims, cfg.eps, cfg.gauge_seed)
-    b = inputs.source_half(sample_dims, cfg.Ls, cfg.source_seed, parity=1)
-    orc = Oracle(sample_dims, cfg.Ls, cfg.M5, cfg.mf, cfg.b5, cfg.c5, antiperiodic_t=cfg.antiperiodic_t,
-                 cut=cfg.cut).set_gauge(U)
-    n5h = b.shape[0] * cfg.Ls
-    for _ in range(warmup):
-        cg(orc, b, 1e-300, iters)
+def host_cpu():
+    """CPU model, physical cores and the threads the oracle's OpenMP loops use (SURVEY 8d "Oracle timing")."""
+    model, phys = "unknown", set()
+    try:
+        pid = cid = None
+        for ln in open("/proc/cpuinfo"):
+            k, _, v = ln.partition(":")
+            k, v = k.strip(), v.strip()
+            if k == "model name":
+                model = v
+            elif k == "physical id":
+                pid = v
+            elif k == "core id":
+                cid = v
+            elif not k and pid is not None:
+                phys.add((pid, cid))
+                pid = cid = None
+    except OSError:
+        pass
+    try:
+        avail = len(os.sched_getaffinity(0))
+    except AttributeError:
+        avail = os.cpu_count() or 1
+    threads = int(os.environ.get("OMP_NUM_THREADS", "0") or 0) or avail
+    return {"cpu_model": model, "physical_cores": len(phys) or None, "logical_cpus": os.cpu_count(), "threads": threads}
+
+
+def _timed(fn, warm, reps):
+    for _ in range(warm):
+        fn()
     t0 = time.perf_counter()
-    for _ in range(steps):
-        cg(orc, b, 1e-300, iters)
-    dt = (time.perf_counter() - t0) / max(steps, 1)
-    return segment_flops(n5h, iters) / dt / 1e9, dt, n5h
+    for _ in range(reps):
+        fn()
+    return (time.perf_counter() - t0) / max(reps, 1)
+
+
+def oracle_setup(cfg, dims, U=None, b=None):
+    from oracle.dwf_oracle import Oracle
+    from paper_2203_17119_b200 import inputs
+    if U is None:
+        U = inputs.gauge_weak(dims, cfg.eps, cfg.gauge_seed)
+    if b is None:
+        b = inputs.source_half(dims, cfg.Ls, cfg.source_seed, parity=1)
+    orc = Oracle(dims, cfg.Ls, cfg.M5, cfg.mf, cfg.b5, cfg.c5, antiperiodic_t=cfg.antiperiodic_t, cut=cfg.cut).set_gauge(U)
+    return orc, b
+
+
+def oracle_workload_baseline(cfg, U, b, iters=1):
+    """cpu_baseline of the own arm: the oracle, as it stands, on the WORKLOAD ITSELF (same lattice, gauge field and source
+    the GPU step ran on): one Dhop (1 warm-up + 3 repetitions), one Mpc^dag Mpc (1 + 2) and one CG segment of `iters`
+    iteration(s) with |b|^2 and the closing true residual (1 repetition, after the warm-ups above)."""
+    from oracle.dwf_oracle import cg
+    orc, b = oracle_setup(cfg, cfg.dims, U, b)
+    n5h = b.shape[0] * cfg.Ls
+    t_dhop = _timed(lambda: orc.dhop(b, 0, False), 1, 3)
+    t_mdagm = _timed(lambda: orc.mdagm(b), 1, 2)
+    t_seg = _timed(lambda: cg(orc, b, 1e-300, iters), 0, 1)
+    return {"value": segment_flops(n5h, iters) / t_seg / 1e9, "unit": UNIT, "kind": "oracle", "s_per_step": t_seg,
+            "dhop_s": t_dhop, "dhop_gflops": FLOP_DHOP * n5h / t_dhop / 1e9,
+            "mdagm_s": t_mdagm, "mdagm_gflops": 2 * FLOP_MPC * n5h / t_mdagm / 1e9,
+            "sample": f"the workload itself ({'x'.join(map(str, cfg.dims))} x Ls={cfg.Ls}, the GPU step's gauge field and source): "
+                      f"half-volume Dhop 1+3 repetitions, Mpc^dag Mpc 1+2, one CG segment of {iters} iteration(s) + |b|^2 + closing "
+                      f"true residual (the GPU step runs 10 iterations per segment); oracle built -O3 -march=native -fno-fast-math"}
 
 
 def run_reference(args, cfg):
+    """--impl reference: the oracle on the host cores.  A step is the CG segment (`--ref-iters` iteration(s) + |b|^2 + closing
+    true residual) on the workload's own lattice when (steps + warmup) such segments fit in ~4 minutes, else on the same
+    lattice shortened in t (same parameters, seeds and recipe); one oracle Dhop on a 32^3 x 4 slab calibrates the choice."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
-    sample = tuple(args.ref_dims)
-    cores = os.cpu_count()
-    val, dt, n5h = oracle_segment(sample, cfg, args.ref_iters, args.steps, args.warmup)
-    desc = (f"oracle CG segment ({args.ref_iters} iteration(s) + closing true residual) on a "
-            f"{'x'.join(map(str, sample))} x Ls={cfg.Ls} sample of {cfg.name} (same parameters, seeds and recipe)")
+    from oracle.dwf_oracle import cg
+    cpu = host_cpu()
+    if args.ref_dims:
+        sample = tuple(args.ref_dims)
+    else:
+        cal = tuple(cfg.dims[:3]) + (4,)
+        orc, b = oracle_setup(cfg, cal)
+        t_cal = _timed(lambda: orc.dhop(b, 0, False), 1, 2)
+        # a 1-iteration segment costs ~17 half-volume Dhops (2 Mpc^dag Mpc + numpy vector work); measured, DESIGN.md section 7
+        per_t = 17.0 * t_cal / 4.0 * (args.ref_iters + 1) / 2.0
+        lt = cfg.dims[3]
+        while lt > 4 and (args.steps + args.warmup) * per_t * lt > 240.0:
+            lt //= 2
+        sample = tuple(cfg.dims[:3]) + (lt,)
+        del orc, b
+    orc, b = oracle_setup(cfg, sample)
+    n5h = b.shape[0] * cfg.Ls
+    dt = _timed(lambda: cg(orc, b, 1e-300, args.ref_iters), args.warmup, args.steps)
+    val = segment_flops(n5h, args.ref_iters) / dt / 1e9
+    desc = (f"oracle CG segment ({args.ref_iters} iteration(s) + |b|^2 + closing true residual) on "
+            f"{'the workload lattice itself' if sample == tuple(cfg.dims) else 'a ' + 'x'.join(map(str, sample)) + ' sample of the workload lattice'}"
+            f" ({'x'.join(map(str, sample))} x Ls={cfg.Ls}, same parameters, seeds and recipe); oracle built -O3 -march=native -fno-fast-math")
+    base = {"value": val, "unit": UNIT, "cores": cpu["threads"], "kind": "oracle", "sample": desc, **cpu}
     line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "sample": desc},
-            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+            "cpu_baseline": base,
             "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line), flush=True)
 
@@ -176,7 +245,8 @@ def run_dwf(args, cfg):
     U, b_np = make_inputs(cfg, rank)
     g = api.from_config(cfg, device=f"cuda:{local}")
     g.set_gauge(U)
-    del U
+    if rank != 0 or world != 1 or args.no_cpu:
+        U = None                       # rank 0 at N = 1 keeps the host copy for the cpu_baseline leg
     A = api
     b = g.pack(b_np, A.F64, A.ODD)
     x = g.new_native(A.F64, A.ODD)
@@ -223,18 +293,34 @@ def run_dwf(args, cfg):
     dhop_avg_ms = dhop_ms / max(dhop_n, 1)
     dhop_bytes = dhop_bytes_total / max(dhop_n, 1)
     achieved = dhop_bytes / (dhop_avg_ms * 1e-3) / 1e9
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "dhop_traffic.csv")       # ncu DRAM bytes per launch (profiles/r01d_dhop.md)
-    if os.path.exists(tp):
-        import csv
-        for row in csv.DictReader(open(tp)):
-            if row["kernel"] == "dhop_f64":
-                traffic = float(row["dram_bytes_per_launch"])
-    roofline = {"bound": "hbm", "kernel": "dhop_tma_kernel<double> (half-volume, 12-real links; per CG iteration 3 plain launches + 1 with the fused Mee epilogue)",
+    traffic64, traffic_src = static_traffic("dhop_f64")
+    roofline = {"bound": "hbm", "dtype": "f64",
+                "kernel": "dhop_tma_kernel<double> (half-volume, 12-real links; per CG iteration 3 plain launches + 1 with the fused Mee epilogue)",
                 "achieved": achieved, "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / hbm_peak,
-                "traffic": traffic, "algorithmic_bytes_per_launch": dhop_bytes, "avg_launch_ms": dhop_avg_ms,
-                "launches_timed": int(dhop_n), "share_of_step": dhop_ms / ms if ms > 0 else None,
+                "traffic": traffic64, "traffic_source": traffic_src, "algorithmic_bytes_per_launch": dhop_bytes,
+                "avg_launch_ms": dhop_avg_ms, "launches_timed": int(dhop_n), "share_of_step": dhop_ms / ms if ms > 0 else None,
                 "gflops": FLOP_DHOP * n5h / (dhop_avg_ms * 1e-3) / 1e9}
+
+    # ---- the same per-launch event timing for the fp32 kernel, inside a long fp32 step with the CG's launch mix (3 plain
+    # + 1 fused Dhop per Mpc^dag Mpc): Chebyshev recurrences of Mpc^dag Mpc in fp32 (dwf_chebyshev, order = 2 x cg-iters)
+    src32 = g.convert(b, A.F64, A.F32, A.ODD)
+    out32 = g.new_native(A.F32, A.ODD)
+    for _ in range(3):
+        g.chebyshev(src32, 0.0, 200.0, 2 * iters, A.F32, out=out32)
+    g.set_option("time_dhop", 1)
+    torch.cuda.synchronize()
+    for _ in range(args.steps):
+        g.chebyshev(src32, 0.0, 200.0, 2 * iters, A.F32, out=out32)
+    ms32, n32, by32 = g.get_option("dhop_ms"), g.get_option("dhop_timed"), g.get_option("dhop_bytes")
+    g.set_option("time_dhop", 0)
+    del src32, out32
+    avg32, b32 = ms32 / max(n32, 1), by32 / max(n32, 1)
+    traffic32, traffic32_src = static_traffic("dhop_f32")
+    roofline_f32 = {"bound": "hbm", "dtype": "f32", "kernel": "dhop_tma_kernel<float> (same launch mix, inside fp32 Chebyshev steps of Mpc^dag Mpc)",
+                    "achieved": b32 / (avg32 * 1e-3) / 1e9, "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s",
+                    "frac": b32 / (avg32 * 1e-3) / 1e9 / hbm_peak, "traffic": traffic32, "traffic_source": traffic32_src,
+                    "algorithmic_bytes_per_launch": b32, "avg_launch_ms": avg32, "launches_timed": int(n32),
+                    "gflops": FLOP_DHOP * n5h / (avg32 * 1e-3) / 1e9}
 
     # ---- e2e: the same step through the C ABI with pinned HOST buffers
     b_host = torch.from_numpy(np.ascontiguousarray(b_np).view(np.float64).reshape(-1)).pin_memory()
@@ -259,23 +345,32 @@ def run_dwf(args, cfg):
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "impl": "dwf",
             "config": {"workload": workload_name(cfg), "step": f"dwf_cg fp64 segment: {iters} iterations + |b|^2 + closing true residual",
-                       "l2": "inputs_larger_than_L2 (each half field 1.2 GB, gauge 0.4 GB per parity)", "parallelism": f"independent subdomains x{world}"},
-            "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "e2e": e2e}
+                       "l2": "inputs_larger_than_L2 (each half field 1.2 GB, gauge 0.4 GB per parity)", "parallelism": f"replicas x{world}: one seeded {cfg.name} subdomain per GPU, no data-path collective"},
+            "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "roofline_f32": roofline_f32, "e2e": e2e}
 
     if rank == 0 and not args.no_extras:
         line["sweeps"] = sweeps(torch, g, A, cfg, hbm_peak)
         line["cg"] = cg_solutions(g, A, b, cfg, args)
     if rank == 0 and world == 1 and not args.no_cpu:
-        sample = tuple(args.ref_dims)
-        val, dt, _ = oracle_segment(sample, cfg, args.ref_iters, 2, 1)
-        line["cpu_baseline"] = {"value": val, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "s_per_step": dt,
-                                "sample": f"oracle CG segment ({args.ref_iters} iteration(s) + closing true residual) on a "
-                                          f"{'x'.join(map(str, sample))} x Ls={cfg.Ls} sample of {cfg.name}, 2 timed repetitions"}
+        cpu = host_cpu()
+        line["cpu_baseline"] = {**oracle_workload_baseline(cfg, U, b_np, args.ref_iters), "cores": cpu["threads"], **cpu}
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(line), flush=True)
+
+
+def static_traffic(kernel):
+    """ncu DRAM bytes per launch of the Dhop kernels: NOT measured in this run -- read from the committed ncu summary
+    (profiles/dhop_traffic.csv names the capture and the commit it was taken at); null when the file has no row."""
+    tp = os.path.join(ROOT, "profiles", "dhop_traffic.csv")
+    if os.path.exists(tp):
+        import csv
+        for row in csv.DictReader(open(tp)):
+            if row["kernel"] == kernel:
+                return float(row["dram_bytes_per_launch"]), f"static: profiles/dhop_traffic.csv ({row.get('capture', 'ncu --set full')})"
+    return None, "none"
 
 
 def sweeps(torch, g, A, cfg, hbm_peak):
@@ -322,7 +417,8 @@ def main():
     ap.add_argument("--workload", default="c4")
     ap.add_argument("--cg-iters", type=int, default=10)
     ap.add_argument("--max-iter", type=int, default=20000)
-    ap.add_argument("--ref-dims", type=int, nargs=4, default=[16, 16, 16, 16])
+    ap.add_argument("--ref-dims", type=int, nargs=4, default=None,
+                    help="reference arm: sample lattice (default: the workload lattice, shortened in t to fit ~4 minutes)")
     ap.add_argument("--ref-iters", type=int, default=1)
     ap.add_argument("--no-extras", action="store_true", help="skip the kernel sweeps and CG time-to-solution")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")

@@ -76,16 +76,14 @@ dwf_status dwf_destroy(dwf_ctx* ctx);
  *   "antiperiodic_t" 0/1 (default 1)       "compress12" 0/1 (default 1; 2-row links, reading C10)
  *   "tile_x","tile_y","tile_z","tile_t"    native tile extents (default 4, or 2 where 4 does not divide)
  *   "inner_tol" (default 1e-4), "max_restarts" (default 20)     mixed-precision CG (reading C9), any time
- *   "dhop_sc" s-slices per thread in the Dhop kernel, "dhop_loop_s" 0/1, any time (tuning)
  *   "time_dhop" 0/1: bracket every Dhop kernel launch with CUDA events on the context stream (restarts the
  *   accumulators); dwf_get_option "dhop_ms" / "dhop_timed" / "dhop_bytes" then synchronise and return the summed
  *   kernel time, the number of launches timed and their summed algorithmic bytes (bench.py's roofline figure)
  *   "fuse" 0/1 (default 1), any time: Mpc / CG use the Dhop kernel's fused Mee epilogue and the streaming CG column
  *   kernels where the TMA Dhop kernel applies (4^4 tiles, 2-row links); get "fused_active" tells whether they do
- *   "dhop_kernel" 0 auto / 1 shape-generic / 2 cp.async tile kernel, "dhop_grid" CTAs of the persistent TMA kernel,
- *   "dhop_order" / "dhop_order_axes" tile traversal (blob extents / path axes as decimal digits),
- *   "dhop_dynamic" 0 static round-robin / 1 global in-order queue: tuning, any time.  "dhop_skip" is a measurement aid
- *   (bit r: halo region r is not loaded; results are then WRONG) and must stay 0 otherwise. */
+ *   "dhop_kernel" 0 auto / 1 shape-generic / 2 cp.async tile kernel and "dhop_dynamic" 0 static round-robin / 1 global
+ *   in-order tile queue select among code paths that compute the same result (used by the parity tests), any time.
+ *   Unknown keys return DWF_EINVAL. */
 dwf_status dwf_set_option(dwf_ctx* ctx, const char* key, double val);
 dwf_status dwf_get_option(const dwf_ctx* ctx, const char* key, double* val);
 /* cudaStream_t as void* (torch.cuda.current_stream().cuda_stream); NULL = default stream */
@@ -128,9 +126,34 @@ dwf_status dwf_norm2(dwf_ctx* ctx, const void* v_dev, dwf_prec prec, dwf_parity 
 
 /* CG on Mpc^dag Mpc x = b (reading C8; mixed: C9).  x_dev: in = initial guess (use_guess != 0) else ignored,
  * out = solution; both fp64 native ODD fields.  tol is relative to |b|.  Restarts from the true residual
- * until |b - A x| <= tol |b|.  Returns DWF_ENOTCONV if max_iter is reached. */
+ * until |b - A x| <= tol |b|.  Returns DWF_ENOTCONV if max_iter is reached.  The stopping test is evaluated on the device
+ * and the host enqueues one iteration ahead of the residual it has read: info->launches may include the kernels of one
+ * iteration past the last counted one, which leave x untouched (x is exactly the iterate of iteration iters_total). */
 dwf_status dwf_cg(dwf_ctx* ctx, void* x_dev, const void* b_dev, double tol, int max_iter, dwf_cg_mode mode,
                   int use_guess, dwf_cg_info* info);
+/* ---- Batched ("multi right-hand side") fields and operators ("four PV local solves, and
+ * two non-local light quark solves" per force evaluation: the Hasenbusch / Pauli-Villars terms are solves with
+ * the same operator on other sources).  N <= 16 systems that share the context's gauge field and parameters are kept in ONE
+ * native half field whose fifth dimension is N * Ls long (slice rhs * Ls + s): dwf_mrhs_field_bytes bytes, device memory
+ * owned by the caller; dwf_mrhs_insert / dwf_mrhs_extract copy system j from / to an ordinary native half field of the same
+ * precision and parity.  The Dhop kernel then loads the 8 links of a site once for N * Ls slices (algorithmic bytes per 5-D
+ * site: 48 B + 8 g B / (N Ls), g = 12 or 18 reals, B = 4 or 8), and every other kernel of Mpc / CG runs once for the whole
+ * batch.  dwf_cg_mrhs runs N independent CGs (readings C8 / C9 per system: own alpha, beta, stopping test, restarts) that
+ * share the launches; a system that has converged is frozen while the others go on.  info: array of nrhs entries.
+ * dwf_mrhs_reserve allocates the batched solver workspace (10 batched half fields per precision) ahead of time; otherwise
+ * the first batched Mpc / CG call with a larger nrhs does.  Status codes as the single-system calls (dwf_cg_mrhs:
+ * DWF_ENOTCONV if any system has not converged at max_iter iterations).  out_parity: DWF_EVEN or DWF_ODD. */
+dwf_status dwf_mrhs_reserve(dwf_ctx* ctx, int nrhs);
+size_t dwf_mrhs_field_bytes(const dwf_ctx* ctx, int nrhs, dwf_prec prec);
+dwf_status dwf_mrhs_insert(dwf_ctx* ctx, void* batched_dev, int nrhs, int j, const void* single_dev, dwf_prec prec);
+dwf_status dwf_mrhs_extract(dwf_ctx* ctx, void* single_dev, const void* batched_dev, int nrhs, int j, dwf_prec prec);
+dwf_status dwf_dhop_mrhs(dwf_ctx* ctx, void* out_dev, const void* in_dev, int nrhs, dwf_parity out_parity, int dagger,
+                         dwf_prec prec);
+dwf_status dwf_mpc_mrhs(dwf_ctx* ctx, void* out_dev, const void* in_dev, int nrhs, int dagger, dwf_prec prec);
+dwf_status dwf_mdagm_mrhs(dwf_ctx* ctx, void* out_dev, const void* in_dev, int nrhs, dwf_prec prec);
+dwf_status dwf_cg_mrhs(dwf_ctx* ctx, void* x_dev, const void* b_dev, int nrhs, double tol, int max_iter, dwf_cg_mode mode,
+                       int use_guess, dwf_cg_info* info);
+
 /* Multishift CG (the solver behind rational functions of D^dag D in the DD-RHMC one-flavour action,
  * eqs. 20-21): (Mpc^dag Mpc + shifts[i]) x_i = b for i < nshift with one shared Krylov space, fp64.
  * x_dev: OUT, nshift fp64 native ODD fields back to back (field i at byte offset i * dwf_field_bytes(F64, ODD)), start

@@ -29,6 +29,8 @@ SYMBOLS = [
     "dwf_field_bytes", "dwf_pack", "dwf_unpack", "dwf_convert", "dwf_dhop", "dwf_meooe5d", "dwf_mooee",
     "dwf_mooee_inv", "dwf_m", "dwf_mpc", "dwf_mdagm", "dwf_norm2", "dwf_cg", "dwf_multishift_cg", "dwf_chebyshev", "dwf_domain_project", "dwf_boundary_op", "dwf_solve", "dwf_dhop_host",
     "dwf_mdagm_host", "dwf_cg_host", "dwf_solve_host", "dwf_launch_count", "dwf_last_error", "dwf_version",
+    "dwf_mrhs_reserve", "dwf_mrhs_field_bytes", "dwf_mrhs_insert", "dwf_mrhs_extract", "dwf_dhop_mrhs", "dwf_mpc_mrhs",
+    "dwf_mdagm_mrhs", "dwf_cg_mrhs",
 ]
 
 
@@ -89,6 +91,15 @@ def load_library():
     lib.dwf_mdagm_host.argtypes = [vp, vp, vp, ci]
     lib.dwf_solve_host.argtypes = [vp, vp, vp, cd, ci, ci, P(CgInfo)]
     lib.dwf_cg_host.argtypes = [vp, vp, vp, cd, ci, ci, P(CgInfo)]
+    lib.dwf_mrhs_reserve.argtypes = [vp, ci]
+    lib.dwf_mrhs_field_bytes.argtypes = [vp, ci, ci]
+    lib.dwf_mrhs_field_bytes.restype = ctypes.c_size_t
+    lib.dwf_mrhs_insert.argtypes = [vp, vp, ci, ci, vp, ci]
+    lib.dwf_mrhs_extract.argtypes = [vp, vp, vp, ci, ci, ci]
+    lib.dwf_dhop_mrhs.argtypes = [vp, vp, vp, ci, ci, ci, ci]
+    lib.dwf_mpc_mrhs.argtypes = [vp, vp, vp, ci, ci, ci]
+    lib.dwf_mdagm_mrhs.argtypes = [vp, vp, vp, ci, ci]
+    lib.dwf_cg_mrhs.argtypes = [vp, vp, vp, ci, cd, ci, ci, ci, P(CgInfo)]
     lib.dwf_launch_count.argtypes = [vp]
     lib.dwf_launch_count.restype = ctypes.c_longlong
     lib.dwf_last_error.argtypes = [vp]
@@ -262,6 +273,55 @@ class Dwf:
         st = self._chk(self.lib.dwf_cg(self._h, self._p(x), self._p(b), tol, max_iter, mode, int(use_guess),
                                        ctypes.byref(info)), allow=(ENOTCONV,))
         return x, info.as_dict(), st
+
+    # ---- batched (multi right-hand side) fields: SURVEY 8f NEXT-3 ---------------------------------
+    def mrhs_reserve(self, nrhs):
+        self._chk(self.lib.dwf_mrhs_reserve(self._h, int(nrhs)))
+
+    def new_mrhs(self, nrhs, prec=F64):
+        nb = self.lib.dwf_mrhs_field_bytes(self._h, int(nrhs), prec)
+        return torch.empty(nb // (8 if prec == F64 else 4), dtype=_rdtype(prec), device=self.device)
+
+    def mrhs_gather(self, fields, prec=F64):
+        """list of native half fields -> one batched field"""
+        n = len(fields)
+        out = self.new_mrhs(n, prec)
+        for j, f in enumerate(fields):
+            self._chk(self.lib.dwf_mrhs_insert(self._h, self._p(out), n, j, self._p(f), prec))
+        return out
+
+    def mrhs_scatter(self, batched, nrhs, prec=F64):
+        """one batched field -> list of native half fields"""
+        outs = []
+        for j in range(nrhs):
+            f = self.new_native(prec, ODD)
+            self._chk(self.lib.dwf_mrhs_extract(self._h, self._p(f), self._p(batched), nrhs, j, prec))
+            outs.append(f)
+        return outs
+
+    def dhop_mrhs(self, inp, nrhs, out_parity, dagger=False, prec=F64, out=None):
+        out = self.new_mrhs(nrhs, prec) if out is None else out
+        self._chk(self.lib.dwf_dhop_mrhs(self._h, self._p(out), self._p(inp), int(nrhs), out_parity, int(dagger), prec))
+        return out
+
+    def mpc_mrhs(self, inp, nrhs, dagger=False, prec=F64, out=None):
+        out = self.new_mrhs(nrhs, prec) if out is None else out
+        self._chk(self.lib.dwf_mpc_mrhs(self._h, self._p(out), self._p(inp), int(nrhs), int(dagger), prec))
+        return out
+
+    def mdagm_mrhs(self, inp, nrhs, prec=F64, out=None):
+        out = self.new_mrhs(nrhs, prec) if out is None else out
+        self._chk(self.lib.dwf_mdagm_mrhs(self._h, self._p(out), self._p(inp), int(nrhs), prec))
+        return out
+
+    def cg_mrhs(self, b, nrhs, tol, max_iter, mode=CG_F64, x=None, use_guess=None):
+        """nrhs independent CGs on a batched fp64 ODD field.  Returns (x batched, [info dict per system], status)."""
+        use_guess = (x is not None) if use_guess is None else bool(use_guess)
+        x = self.new_mrhs(nrhs, F64) if x is None else x
+        infos = (CgInfo * nrhs)()
+        st = self._chk(self.lib.dwf_cg_mrhs(self._h, self._p(x), self._p(b), int(nrhs), tol, max_iter, mode, int(use_guess),
+                                            infos), allow=(ENOTCONV,))
+        return x, [i.as_dict() for i in infos], st
 
     def domain_project(self, inp, which, prec=F64, out=None):
         """which = 0: P_Omega, 1: P_Omegabar, 2: boundary projector P_dbar; FULL native fields."""

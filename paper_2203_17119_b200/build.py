@@ -33,6 +33,17 @@ def _deps_mtime() -> float:
     return max(os.path.getmtime(p) for p in paths)
 
 
+def _flags() -> list:
+    """DWF_PROBE=1 in the environment compiles the measurement knobs in (tile order, grid size, halo skipping ...:
+    dwf_set_option keys the product build rejects); the product build is the one without it."""
+    return NVCC_FLAGS + (["-DDWF_PROBE"] if os.environ.get("DWF_PROBE", "0") not in ("", "0") else [])
+
+
+def _stamp_ok() -> bool:
+    p = os.path.join(BUILD, "flags.txt")
+    return os.path.exists(p) and open(p).read() == " ".join(_flags())
+
+
 def _compile(src: str, verbose: bool) -> str:
     obj = os.path.join(BUILD, src.replace(".cu", ".o"))
     srcp = os.path.join(CSRC, src)
@@ -40,7 +51,7 @@ def _compile(src: str, verbose: bool) -> str:
     hdr_m = max(hdr_m, os.path.getmtime(os.path.join(HERE, "..", "include", "dwf.h")))
     if os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(srcp), hdr_m):
         return obj
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", srcp, "-o", obj]
+    cmd = [_nvcc()] + _flags() + (["-Xptxas", "-v"] if verbose else []) + ["-c", srcp, "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if verbose:
         sys.stderr.write(r.stderr)
@@ -51,6 +62,8 @@ def _compile(src: str, verbose: bool) -> str:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(BUILD, exist_ok=True)
+    if not _stamp_ok():
+        force = True
     if force:
         for f in os.listdir(BUILD):
             if f.endswith(".o"):
@@ -63,6 +76,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
+    with open(os.path.join(BUILD, "flags.txt"), "w") as f:
+        f.write(" ".join(_flags()))
     return LIB
 
 

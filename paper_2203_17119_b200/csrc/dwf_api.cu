@@ -17,15 +17,51 @@ namespace {
 
 const int NWS = 10;
 
-dwf_status ws_get(dwf_ctx* c, int prec, int idx, void** out) {
-    void** arr = (prec == DWF_F64) ? c->ws64 : c->ws32;
-    if (!arr[idx]) {
-        if (cudaMalloc(&arr[idx], half_bytes(c->g, prec)) != cudaSuccess) {
-            c->err = "cudaMalloc(workspace) failed";
-            cudaGetLastError();
-            return DWF_ENOMEM;
-        }
+// The solver workspace (NWS half fields per precision) is allocated once, at dwf_set_gauge: no operator, dwf_cg or
+// dwf_solve call allocates device memory ("ctx owns ... CG workspace; no allocation inside dwf_cg").
+// The batched (multi right-hand side) calls have their own set, sized by dwf_mrhs_reserve (or by the first batched call).
+dwf_status ws_alloc_all(dwf_ctx* c) {
+    for (int prec = 0; prec < 2; ++prec) {
+        void** arr = (prec == DWF_F64) ? c->ws64 : c->ws32;
+        for (int i = 0; i < NWS; ++i)
+            if (!arr[i] && cudaMalloc(&arr[i], half_bytes(c->g, prec)) != cudaSuccess) {
+                c->err = "cudaMalloc(workspace) failed";
+                cudaGetLastError();
+                return DWF_ENOMEM;
+            }
     }
+    return DWF_OK;
+}
+
+void wsm_free(dwf_ctx* c) {
+    for (int i = 0; i < NWS; ++i) {
+        if (c->wsm64[i]) cudaFree(c->wsm64[i]);
+        if (c->wsm32[i]) cudaFree(c->wsm32[i]);
+        c->wsm64[i] = c->wsm32[i] = nullptr;
+    }
+    c->mrhs_cap = 0;
+}
+
+dwf_status wsm_reserve(dwf_ctx* c, int nrhs) {
+    if (nrhs <= c->mrhs_cap) return DWF_OK;
+    wsm_free(c);
+    for (int prec = 0; prec < 2; ++prec) {
+        void** arr = (prec == DWF_F64) ? c->wsm64 : c->wsm32;
+        for (int i = 0; i < NWS; ++i)
+            if (cudaMalloc(&arr[i], half_bytes(c->g, prec) * nrhs) != cudaSuccess) {
+                cudaGetLastError();
+                wsm_free(c);
+                c->err = "cudaMalloc(batched workspace) failed";
+                return DWF_ENOMEM;
+            }
+    }
+    c->mrhs_cap = nrhs;
+    return DWF_OK;
+}
+
+dwf_status ws_get(dwf_ctx* c, int prec, int idx, void** out) {
+    void** arr = (c->nrhs_cur > 1) ? ((prec == DWF_F64) ? c->wsm64 : c->wsm32) : ((prec == DWF_F64) ? c->ws64 : c->ws32);
+    if (!arr[idx] || (c->nrhs_cur > 1 && c->nrhs_cur > c->mrhs_cap)) { c->err = "workspace not allocated (call dwf_set_gauge)"; return DWF_ESTATE; }
     *out = arr[idx];
     return DWF_OK;
 }
@@ -42,12 +78,23 @@ dwf_status need_gauge(dwf_ctx* c) {
     return DWF_OK;
 }
 
+// sizes of ONE system's half field, and of the field the call in progress works on (all c->nrhs_cur systems)
 size_t half_reals(const dwf_ctx* c) { return (size_t)c->g.Vh * c->g.Ls * 24; }
+size_t cur_bytes(const dwf_ctx* c, int prec) { return half_bytes(c->g, prec) * c->nrhs_cur; }
 
-dwf_status read_slot(dwf_ctx* c, int slot, double* v) {
-    DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->scalars_host + slot, c->scalars + slot, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+// scalars[slot][0 .. nrhs_cur) -> host (synchronises the stream)
+dwf_status read_slots(dwf_ctx* c, int slot, double* v) {
+    const size_t o = (size_t)slot * MAXR;
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->scalars_host + o, c->scalars + o, sizeof(double) * c->nrhs_cur, cudaMemcpyDeviceToHost, c->stream));
     DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
-    *v = c->scalars_host[slot];
+    for (int j = 0; j < c->nrhs_cur; ++j) v[j] = c->scalars_host[o + j];
+    return DWF_OK;
+}
+dwf_status read_slot(dwf_ctx* c, int slot, double* v) {      // system 0 only
+    const size_t o = (size_t)slot * MAXR;
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->scalars_host + o, c->scalars + o, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    *v = c->scalars_host[o];
     return DWF_OK;
 }
 
@@ -107,69 +154,120 @@ dwf_status m_apply(dwf_ctx* c, void* out, const void* in, int dagger, int prec) 
     return DWF_OK;
 }
 
-// CG iterations on A = Mpc^dag Mpc in precision prec.  On entry r holds the residual, slot_c |r|^2 (host copy cval).
-// Mirrors the oracle's loop order (reading C8).  Returns the number of iterations done and the last |r|^2.
-dwf_status cg_iterate(dwf_ctx* c, int prec, void* x, void* r, double target, int max_iter, int* iters_io, double* cval) {
-    void *p, *q, *z;
+// ---- CG on A = Mpc^dag Mpc for the c->nrhs_cur systems of a (batched) field (readings C8, C9) ------------------------
+// The stopping test lives on the device (reduce_partials_kernel: cg_conv[j] = first iteration with |r_j|^2 <= cg_target[j])
+// and the host enqueues iteration k + 1 before it has read the residual of iteration k: the GPU never waits for the host.
+// Iteration k + 1 of a system that stopped at k only touches work vectors (cg_xp / cg_update leave x and p alone), so the
+// solution is the iterate of iteration k exactly, and the iteration count reported is k -- as in the oracle's loop.
+struct CgRun {
+    int n;                       // systems
+    double target[MAXR];         // tol^2 |b|^2 (or the inner target), per system
+    double c[MAXR];              // in: |r|^2 on entry; out: |r|^2 at the system's last counted iteration
+    int iters[MAXR];             // out: iterations counted for the system in this run
+    int launched;                // out: iterations enqueued (>= max iters[]: at most one more)
+};
+
+dwf_status cg_upload_state(dwf_ctx* c, CgRun& run, int slot_c) {
+    double* h = c->scalars_host;
+    int* hconv = reinterpret_cast<int*>(c->cn_ring + (size_t)CG_RING * MAXR + MAXR);
+    double* htgt = c->cn_ring + (size_t)CG_RING * MAXR;
+    for (int j = 0; j < run.n; ++j) {
+        h[(size_t)slot_c * MAXR + j] = run.c[j];
+        htgt[j] = run.target[j];
+        hconv[j] = (run.c[j] <= run.target[j]) ? 0 : -1;          // already there: frozen from the start
+    }
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->scalars + (size_t)slot_c * MAXR, h + (size_t)slot_c * MAXR, sizeof(double) * run.n, cudaMemcpyHostToDevice, c->stream));
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->cg_target, htgt, sizeof(double) * run.n, cudaMemcpyHostToDevice, c->stream));
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->cg_conv, hconv, sizeof(int) * run.n, cudaMemcpyHostToDevice, c->stream));
+    DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));        // the pinned staging is reused by the next upload
+    return DWF_OK;
+}
+
+// On entry r holds the residuals and run.c their |.|^2; at most max_iter iterations are counted for any system.
+dwf_status cg_iterate(dwf_ctx* c, int prec, void* x, void* r, int max_iter, CgRun& run) {
+    void *p, *q, *z, *t1 = nullptr, *t2 = nullptr;
     DWF_TRY(ws_get(c, prec, 3, &p));
     DWF_TRY(ws_get(c, prec, 4, &q));
     DWF_TRY(ws_get(c, prec, 5, &z));
+    DWF_TRY(ws_get(c, prec, 0, &t1));
+    DWF_TRY(ws_get(c, prec, 1, &t2));
     const size_t n = half_reals(c);
+    const int N = run.n;
     int slot_c = SLOT_C, slot_cn = SLOT_CN;
-    double cc = *cval;
-    if (dhop_fused_available(c)) {
-        // 8 kernels per iteration moving 23 half fields instead of 11 moving 29: the second Dhop
-        // carries q = Mee p - 1/4 (..) and |q|^2; one column kernel forms z = Mpc^dag's last step in registers and does
-        // r -= alpha z, |r|^2; one does x += alpha p, p = r + beta p and the next A p.  Same operation order as the
-        // unfused loop (reading C8).
-        void *t1, *t2;
-        DWF_TRY(ws_get(c, prec, 0, &t1));
-        DWF_TRY(ws_get(c, prec, 1, &t2));
-        DWF_TRY(launch_cg_xp(c, x, p, r, t1, prec, slot_c, SLOT_D, slot_cn, 1));          // p = r, t1 = A p
-        while (cc > target && *iters_io < max_iter) {
+    DWF_TRY(cg_upload_state(c, run, slot_c));
+    int conv[MAXR];
+    bool all = true;
+    for (int j = 0; j < N; ++j) {
+        conv[j] = (run.c[j] <= run.target[j]) ? 0 : -1;
+        run.iters[j] = 0;
+        all = all && conv[j] >= 0;
+    }
+    run.launched = 0;
+    if (all || max_iter <= 0) return DWF_OK;
+    const bool fused = dhop_fused_available(c);
+    // 8 kernels per iteration moving 23 half fields when the fused kernels apply: the second Dhop
+    // carries q = Mee p - 1/4 (..) and |q|^2; one column kernel forms z = Mpc^dag's last step in registers and does
+    // r -= alpha z, |r|^2; one does x += alpha p, p = r + beta p and the next A p.  Same operation order as the
+    // unfused loop (reading C8).
+    if (fused) DWF_TRY(launch_cg_xp(c, x, p, r, t1, prec, slot_c, SLOT_D, slot_cn, 1, 0));          // p = r, t1 = A p
+    else DWF_CUDA_CHECK(c, cudaMemcpyAsync(p, r, cur_bytes(c, prec), cudaMemcpyDeviceToDevice, c->stream));
+    int k = 0, decided = 0, stop_at = -1;
+    // reads |r|^2 of iteration `it` (waits for it) and applies the stopping test; returns true when every system has stopped
+    auto decide = [&](int it, dwf_status* st) -> bool {
+        *st = DWF_OK;
+        if (cudaEventSynchronize(c->cg_ev[it % CG_RING]) != cudaSuccess) { c->err = "cudaEventSynchronize failed"; *st = DWF_ECUDA; return true; }
+        const double* cn = c->cn_ring + (size_t)(it % CG_RING) * MAXR;
+        bool done = true;
+        for (int j = 0; j < N; ++j) {
+            if (conv[j] >= 0) continue;
+            if (!(cn[j] == cn[j])) { c->err = "CG: NaN residual"; run.c[j] = cn[j]; *st = DWF_ECUDA; return true; }
+            run.c[j] = cn[j];
+            run.iters[j] = it;
+            if (cn[j] <= run.target[j]) conv[j] = it; else done = false;
+        }
+        decided = it;
+        return done;
+    };
+    dwf_status st = DWF_OK;
+    while (k < max_iter) {
+        ++k;
+        if (fused) {
             DWF_TRY(launch_dhop(c, t2, t1, DWF_EVEN, 0, prec));
             DWF_TRY(launch_op5(c, t1, t2, OP_A_MEEINV, nullptr, -1, 0.0, prec, -1));
             DWF_TRY(launch_dhop_fused(c, q, t1, DWF_ODD, prec, p, -0.25, SLOT_D));           // q = Mpc p, d = |q|^2
             DWF_TRY(launch_dhop(c, t1, q, DWF_EVEN, 1, prec));
             DWF_TRY(launch_op5(c, t2, t1, OP_MEEINVDAG_ADAG, nullptr, -1, 0.0, prec, -1));
             DWF_TRY(launch_dhop(c, t1, t2, DWF_ODD, 1, prec));
-            DWF_TRY(launch_cg_r(c, r, q, t1, -0.25, prec, slot_c, SLOT_D, slot_cn));   // r -= a Mpc^dag q
-            double cn;
-            DWF_TRY(read_slot(c, slot_cn, &cn));
-            ++*iters_io;
-            if (!(cn == cn)) { c->err = "CG: NaN residual"; *cval = cn; return DWF_ECUDA; }
-            DWF_TRY(launch_cg_xp(c, x, p, r, t1, prec, slot_c, SLOT_D, slot_cn, 0));      // x += a p; p = r + b p; t1 = A p
-            cc = cn;
-            if (cn <= target) break;
-            int t = slot_c; slot_c = slot_cn; slot_cn = t;
+            DWF_TRY(launch_cg_r(c, r, q, t1, -0.25, prec, slot_c, SLOT_D, slot_cn, k));     // r -= a Mpc^dag q; stopping test
+        } else {
+            DWF_TRY(mpc_apply(c, q, p, 0, prec, SLOT_D));                 // q = Mpc p, d = |q|^2
+            DWF_TRY(mpc_apply(c, z, q, 1, prec, -1));                     // z = Mpc^dag q
+            DWF_TRY(launch_cg_update(c, x, r, p, z, prec, n, slot_c, SLOT_D, slot_cn, k));   // x += a p; r -= a z; test
         }
-        *cval = cc;
-        return DWF_OK;
+        DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->cn_ring + (size_t)(k % CG_RING) * MAXR, c->scalars + (size_t)slot_cn * MAXR,
+                                          sizeof(double) * N, cudaMemcpyDeviceToHost, c->stream));
+        DWF_CUDA_CHECK(c, cudaEventRecord(c->cg_ev[k % CG_RING], c->stream));
+        if (fused) DWF_TRY(launch_cg_xp(c, x, p, r, t1, prec, slot_c, SLOT_D, slot_cn, 0, k));      // x += a p; p = r + b p; t1 = A p
+        else DWF_TRY(launch_xpay(c, p, r, prec, n, slot_cn, slot_c));                           // p = r + (cn/c) p
+        { int t = slot_c; slot_c = slot_cn; slot_cn = t; }
+        if (k >= 2 && decide(k - 1, &st)) { stop_at = k - 1; break; }
     }
-    DWF_CUDA_CHECK(c, cudaMemcpyAsync(p, r, half_bytes(c->g, prec), cudaMemcpyDeviceToDevice, c->stream));
-    while (cc > target && *iters_io < max_iter) {
-        DWF_TRY(mpc_apply(c, q, p, 0, prec, SLOT_D));                 // q = Mpc p, d = |q|^2
-        DWF_TRY(mpc_apply(c, z, q, 1, prec, -1));                     // z = Mpc^dag q
-        DWF_TRY(launch_cg_update(c, x, r, p, z, prec, n, slot_c, SLOT_D, slot_cn));
-        double cn;
-        DWF_TRY(read_slot(c, slot_cn, &cn));
-        ++*iters_io;
-        if (!(cn == cn)) { c->err = "CG: NaN residual"; *cval = cn; return DWF_ECUDA; }
-        if (cn <= target) { cc = cn; break; }
-        DWF_TRY(launch_xpay(c, p, r, prec, n, slot_cn, slot_c));      // p = r + (cn/c) p
-        int t = slot_c; slot_c = slot_cn; slot_cn = t;
-        cc = cn;
+    if (st != DWF_OK) return st;
+    while (stop_at < 0 && decided < k) {
+        if (decide(decided + 1, &st)) stop_at = decided;
+        if (st != DWF_OK) return st;
     }
-    *cval = cc;
+    run.launched = k;
     return DWF_OK;
 }
 
+// |v_j|^2 of every system of the field in progress
 dwf_status norm2_host(dwf_ctx* c, const void* v, int prec, double* out) {
     DWF_TRY(launch_norm2(c, v, prec, half_reals(c), SLOT_T0));
-    return read_slot(c, SLOT_T0, out);
+    return read_slots(c, SLOT_T0, out);
 }
 
-// r = b - A x (fp64), returns |r|^2
+// r = b - A x (fp64), returns |r_j|^2
 dwf_status true_residual(dwf_ctx* c, void* r, const void* b, const void* x, double* rn2) {
     void* ax;
     DWF_TRY(ws_get(c, DWF_F64, 6, &ax));
@@ -178,45 +276,67 @@ dwf_status true_residual(dwf_ctx* c, void* r, const void* b, const void* x, doub
     return norm2_host(c, r, DWF_F64, rn2);
 }
 
+// zero the systems of a batched fp64 field whose right-hand side vanishes (x_j = 0 is the solution)
+dwf_status zero_systems(dwf_ctx* c, void* x, const double* bn2) {
+    const size_t chunk = (size_t)c->g.Ls * 12 * c->g.TS * 16;       // bytes of one tile of one system
+    for (int j = 0; j < c->nrhs_cur; ++j)
+        if (bn2[j] == 0.0)
+            DWF_CUDA_CHECK(c, cudaMemset2DAsync((char*)x + j * chunk, chunk * c->nrhs_cur, 0, chunk, c->g.ntiles, c->stream));
+    return DWF_OK;
+}
+
+// info: one entry per system
 dwf_status cg_f64(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, int use_guess, dwf_cg_info* info) {
     void* r;
     DWF_TRY(ws_get(c, DWF_F64, 2, &r));
-    const size_t hb = half_bytes(c->g, DWF_F64);
-    double bn2;
-    DWF_TRY(norm2_host(c, b, DWF_F64, &bn2));
+    const int N = c->nrhs_cur;
+    const size_t hb = cur_bytes(c, DWF_F64);
+    double bn2[MAXR];
+    DWF_TRY(norm2_host(c, b, DWF_F64, bn2));
     if (!use_guess) DWF_CUDA_CHECK(c, cudaMemsetAsync(x, 0, hb, c->stream));
-    if (bn2 == 0.0) {
-        DWF_CUDA_CHECK(c, cudaMemsetAsync(x, 0, hb, c->stream));
-        info->resid_iter = info->resid_true = 0.0;
-        return DWF_OK;
-    }
-    const double target = tol * tol * bn2;
-    int iters = 0, restarts = 0;
-    double cc = 0.0, rtrue = 0.0;
+    else DWF_TRY(zero_systems(c, x, bn2));
+    bool any = false;
+    for (int j = 0; j < N; ++j) any = any || bn2[j] != 0.0;
+    if (!any) return DWF_OK;
+    CgRun run;
+    run.n = N;
+    for (int j = 0; j < N; ++j) run.target[j] = tol * tol * bn2[j];
+    int iters[MAXR] = {}, restarts = 0, launched = 0;
+    double rt[MAXR];
     bool conv = false;
     for (;;) {
         if (use_guess || restarts > 0) {
-            DWF_TRY(true_residual(c, r, b, x, &cc));
+            DWF_TRY(true_residual(c, r, b, x, run.c));
         } else {
             DWF_CUDA_CHECK(c, cudaMemcpyAsync(r, b, hb, cudaMemcpyDeviceToDevice, c->stream));
-            cc = bn2;
+            for (int j = 0; j < N; ++j) run.c[j] = bn2[j];
         }
-        c->scalars_host[SLOT_C] = cc;
-        DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->scalars + SLOT_C, c->scalars_host + SLOT_C, sizeof(double), cudaMemcpyHostToDevice, c->stream));
-        DWF_TRY(cg_iterate(c, DWF_F64, x, r, target, max_iter, &iters, &cc));
-        info->resid_iter = std::sqrt(cc / bn2);
+        DWF_TRY(cg_iterate(c, DWF_F64, x, r, max_iter - launched, run));
+        launched += run.launched;
+        for (int j = 0; j < N; ++j) {
+            iters[j] += run.iters[j];
+            info[j].resid_iter = bn2[j] > 0 ? std::sqrt(run.c[j] / bn2[j]) : 0.0;
+        }
         void* tr;
         DWF_TRY(ws_get(c, DWF_F64, 7, &tr));
-        double tn2;
-        DWF_TRY(true_residual(c, tr, b, x, &tn2));
-        rtrue = std::sqrt(tn2 / bn2);
-        if (rtrue <= tol) { conv = true; break; }
-        if (iters >= max_iter) break;
+        double tn2[MAXR];
+        DWF_TRY(true_residual(c, tr, b, x, tn2));
+        conv = true;
+        for (int j = 0; j < N; ++j) {
+            rt[j] = bn2[j] > 0 ? std::sqrt(tn2[j] / bn2[j]) : 0.0;
+            conv = conv && rt[j] <= tol;
+        }
+        if (conv) break;
+        int most = 0;
+        for (int j = 0; j < N; ++j) most = iters[j] > most ? iters[j] : most;
+        if (most >= max_iter || launched >= max_iter) break;
         ++restarts;
     }
-    info->iters_total = iters;
-    info->restarts = restarts;
-    info->resid_true = rtrue;
+    for (int j = 0; j < N; ++j) {
+        info[j].iters_total = iters[j];
+        info[j].restarts = restarts;
+        info[j].resid_true = rt[j];
+    }
     return conv ? DWF_OK : DWF_ENOTCONV;
 }
 
@@ -226,36 +346,56 @@ dwf_status cg_mixed(dwf_ctx* c, void* x, const void* b, double tol, int max_iter
     DWF_TRY(ws_get(c, DWF_F64, 2, &r));
     DWF_TRY(ws_get(c, DWF_F32, 2, &r32));
     DWF_TRY(ws_get(c, DWF_F32, 6, &e32));
-    const size_t hb = half_bytes(c->g, DWF_F64), hb32 = half_bytes(c->g, DWF_F32);
-    double bn2;
-    DWF_TRY(norm2_host(c, b, DWF_F64, &bn2));
-    if (!use_guess || bn2 == 0.0) DWF_CUDA_CHECK(c, cudaMemsetAsync(x, 0, hb, c->stream));
-    if (bn2 == 0.0) { info->resid_iter = info->resid_true = 0.0; return DWF_OK; }
-    int iters = 0, restarts = 0;
-    double rtrue = 0.0;
+    const int N = c->nrhs_cur;
+    const size_t hb = cur_bytes(c, DWF_F64), hb32 = cur_bytes(c, DWF_F32);
+    double bn2[MAXR];
+    DWF_TRY(norm2_host(c, b, DWF_F64, bn2));
+    if (!use_guess) DWF_CUDA_CHECK(c, cudaMemsetAsync(x, 0, hb, c->stream));
+    else DWF_TRY(zero_systems(c, x, bn2));
+    bool any = false;
+    for (int j = 0; j < N; ++j) any = any || bn2[j] != 0.0;
+    if (!any) return DWF_OK;
+    int iters[MAXR] = {}, restarts = 0, launched = 0, outer[MAXR] = {};
+    double rt[MAXR];
+    bool conv = false;
     for (;;) {
-        double rn2;
-        DWF_TRY(true_residual(c, r, b, x, &rn2));
-        rtrue = std::sqrt(rn2 / bn2);
-        if (rtrue <= tol || restarts >= c->max_restarts || iters >= max_iter) break;
-        const double delta = std::fmax(c->inner_tol, tol * std::sqrt(bn2 / rn2));
+        double rn2[MAXR];
+        DWF_TRY(true_residual(c, r, b, x, rn2));
+        conv = true;
+        for (int j = 0; j < N; ++j) {
+            rt[j] = bn2[j] > 0 ? std::sqrt(rn2[j] / bn2[j]) : 0.0;
+            conv = conv && rt[j] <= tol;
+        }
+        if (conv || restarts >= c->max_restarts || launched >= max_iter) break;
         DWF_TRY(launch_convert(c, r32, DWF_F32, r, DWF_F64, 1));
-        double r32n2;
-        DWF_TRY(norm2_host(c, r32, DWF_F32, &r32n2));
+        CgRun run;
+        run.n = N;
+        DWF_TRY(norm2_host(c, r32, DWF_F32, run.c));
         DWF_CUDA_CHECK(c, cudaMemsetAsync(e32, 0, hb32, c->stream));
-        c->scalars_host[SLOT_C] = r32n2;
-        DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->scalars + SLOT_C, c->scalars_host + SLOT_C, sizeof(double), cudaMemcpyHostToDevice, c->stream));
-        double cc = r32n2;
-        DWF_TRY(cg_iterate(c, DWF_F32, e32, r32, delta * delta * r32n2, max_iter, &iters, &cc));
-        info->resid_iter = std::sqrt(cc / r32n2);
+        double r32n2[MAXR];
+        for (int j = 0; j < N; ++j) {
+            r32n2[j] = run.c[j];
+            if (rt[j] <= tol) { run.target[j] = 1e300; continue; }       // this system is done: frozen, e_j stays 0
+            const double delta = std::fmax(c->inner_tol, tol * std::sqrt(bn2[j] / rn2[j]));
+            run.target[j] = delta * delta * r32n2[j];
+            ++outer[j];
+        }
+        DWF_TRY(cg_iterate(c, DWF_F32, e32, r32, max_iter - launched, run));
+        launched += run.launched;
+        for (int j = 0; j < N; ++j) {
+            iters[j] += run.iters[j];
+            if (r32n2[j] > 0 && rt[j] > tol) info[j].resid_iter = std::sqrt(run.c[j] / r32n2[j]);
+        }
         DWF_TRY(launch_add_f32_to_f64(c, x, e32, 0));
         ++restarts;
     }
-    info->iters_total = iters;
-    info->iters_inner = iters;
-    info->restarts = restarts;
-    info->resid_true = rtrue;
-    return (rtrue <= tol) ? DWF_OK : DWF_ENOTCONV;
+    for (int j = 0; j < N; ++j) {
+        info[j].iters_total = iters[j];
+        info[j].iters_inner = iters[j];
+        info[j].restarts = outer[j];
+        info[j].resid_true = rt[j];
+    }
+    return conv ? DWF_OK : DWF_ENOTCONV;
 }
 
 double now_s() {
@@ -320,16 +460,24 @@ dwf_status dwf_create(dwf_ctx** out, const int dims[4], int Ls, double M5, doubl
     }
     c->g.Ls = Ls;
     c->g.antiperiodic_t = 1;
+    cudaGetDevice(&c->device);
     c->M5 = M5; c->mf = mf; c->b5 = b5; c->c5 = c5;
     choose_tiles(c);
     build_tables(c);
-    if (cudaMalloc(&c->scalars, sizeof(double) * NSLOTS) != cudaSuccess ||
-        cudaMallocHost(&c->scalars_host, sizeof(double) * NSLOTS) != cudaSuccess) {
+    bool ok = cudaMalloc(&c->scalars, sizeof(double) * NSLOTS * MAXR) == cudaSuccess &&
+              cudaMallocHost(&c->scalars_host, sizeof(double) * NSLOTS * MAXR) == cudaSuccess &&
+              cudaMalloc(&c->cg_target, sizeof(double) * MAXR) == cudaSuccess &&
+              cudaMalloc(&c->cg_conv, sizeof(int) * MAXR) == cudaSuccess &&
+              // |r|^2 ring of the last CG_RING iterations, then the staging of cg_target and cg_conv
+              cudaMallocHost(&c->cn_ring, sizeof(double) * (CG_RING + 2) * MAXR) == cudaSuccess &&
+              cudaMemset(c->scalars, 0, sizeof(double) * NSLOTS * MAXR) == cudaSuccess &&
+              cudaMemset(c->cg_conv, 0xff, sizeof(int) * MAXR) == cudaSuccess;
+    for (int i = 0; i < CG_RING && ok; ++i) ok = cudaEventCreateWithFlags(&c->cg_ev[i], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) {
         cudaGetLastError();
-        delete c;
+        dwf_destroy(c);
         return DWF_ECUDA;
     }
-    cudaMemset(c->scalars, 0, sizeof(double) * NSLOTS);
     // device tables [op][chirality][Ls*Ls]
     const size_t nt = (size_t)OP5_COUNT * 2 * Ls * Ls;
     std::vector<double> h64(nt);
@@ -356,6 +504,7 @@ dwf_status dwf_create(dwf_ctx** out, const int dims[4], int Ls, double M5, doubl
 }
 
 dwf_status dwf_destroy(dwf_ctx* c) {
+    DeviceGuard _dev(c);
     if (!c) return DWF_EINVAL;
     for (int p = 0; p < 2; ++p) {
         if (c->W64[p]) cudaFree(c->W64[p]);
@@ -376,6 +525,12 @@ dwf_status dwf_destroy(dwf_ctx* c) {
     if (c->partials) cudaFree(c->partials);
     if (c->scalars) cudaFree(c->scalars);
     if (c->scalars_host) cudaFreeHost(c->scalars_host);
+    if (c->cg_target) cudaFree(c->cg_target);
+    if (c->cg_conv) cudaFree(c->cg_conv);
+    if (c->cn_ring) cudaFreeHost(c->cn_ring);
+    for (int i = 0; i < CG_RING; ++i)
+        if (c->cg_ev[i]) cudaEventDestroy(c->cg_ev[i]);
+    wsm_free(c);
     if (c->dtab.d64) cudaFree(c->dtab.d64);
     if (c->dtab.d32) cudaFree(c->dtab.d32);
     cudaGetLastError();
@@ -384,6 +539,7 @@ dwf_status dwf_destroy(dwf_ctx* c) {
 }
 
 dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
+    DeviceGuard _dev(c);
     if (!c || !key) return DWF_EINVAL;
     const std::string k(key);
     const bool pre_gauge = (k == "antiperiodic_t" || k == "compress12" || k.rfind("tile_", 0) == 0);
@@ -400,19 +556,23 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
         if (c->g.TS > 1024) { c->tile_opt[mu] = old; choose_tiles(c); c->err = "tile too large"; return DWF_EINVAL; }
     } else if (k == "inner_tol") c->inner_tol = val;
     else if (k == "max_restarts") c->max_restarts = (int)val;
+    else if (k == "dhop_kernel") c->dhop_kernel = (int)val;
+    else if (k == "fuse") c->fuse = (val != 0.0);
+    else if (k == "dhop_dynamic") { if (val < 0 || val > 1) return DWF_EINVAL; c->dhop_dynamic = (int)val; }
+#ifdef DWF_PROBE
+    // measurement knobs of the probe build (python -m paper_2203_17119_b200.build with DWF_PROBE=1); not part of the ABI
     else if (k == "dhop_sc") { if (val < 0 || val > 4) return DWF_EINVAL; c->dhop_sc = (int)val; }
     else if (k == "dhop_loop_s") c->dhop_loop_s = (val != 0.0);
-    else if (k == "dhop_kernel") c->dhop_kernel = (int)val;
     else if (k == "dhop_grid") { if (val < 0) return DWF_EINVAL; c->dhop_grid = (int)val; }
     else if (k == "dhop_order" || k == "dhop_order_axes") {
         if (val < 0 || val > 9999) return DWF_EINVAL;
         (k == "dhop_order" ? c->dhop_order : c->dhop_order_axes) = (int)val;
         if (c->gauge_set) DWF_TRY(tma_state_build(c));
     }
-    else if (k == "fuse") c->fuse = (val != 0.0);
     else if (k == "dhop_skip") c->dhop_skip = (int)val;
-    else if (k == "dhop_dynamic") { if (val < 0 || val > 1) return DWF_EINVAL; c->dhop_dynamic = (int)val; }
+    else if (k == "dhop_l2hint") c->dhop_l2hint = (int)val;
     else if (k == "dhop_nst") { if (val != 2 && val != 3) return DWF_EINVAL; c->dhop_nst = (int)val; }
+#endif
     else if (k == "time_dhop") {       // (re)start per-launch event timing of the Dhop kernel
         DWF_TRY(dhop_timing_flush(c));
         c->time_dhop = (val != 0.0);
@@ -425,6 +585,7 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
 }
 
 dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
+    DeviceGuard _dev(c);
     if (!c || !key || !val) return DWF_EINVAL;
     const std::string k(key);
     if (k == "dhop_ms" || k == "dhop_timed" || k == "dhop_bytes") {   // synchronises: folds the pending event pairs
@@ -441,28 +602,25 @@ dwf_status dwf_get_option(const dwf_ctx* c, const char* key, double* val) {
     else if (k == "tile_t") *val = c->g.T[3];
     else if (k == "inner_tol") *val = c->inner_tol;
     else if (k == "max_restarts") *val = c->max_restarts;
-    else if (k == "dhop_sc") *val = c->dhop_sc;
-    else if (k == "dhop_loop_s") *val = c->dhop_loop_s;
     else if (k == "time_dhop") *val = c->time_dhop;
     else if (k == "dhop_kernel") *val = c->dhop_kernel;
-    else if (k == "dhop_nst") *val = c->dhop_nst;
-    else if (k == "dhop_grid") *val = c->dhop_grid;
     else if (k == "dhop_dynamic") *val = c->dhop_dynamic;
     else if (k == "fuse") *val = c->fuse;
     else if (k == "fused_active") *val = dhop_fused_available(c) ? 1.0 : 0.0;
-    else if (k == "dhop_order") *val = c->dhop_order;
-    else if (k == "dhop_order_axes") *val = c->dhop_order_axes;
+    else if (k == "mrhs_reserved") *val = c->mrhs_cap;
     else return DWF_EINVAL;
     return DWF_OK;
 }
 
 dwf_status dwf_set_stream(dwf_ctx* c, void* s) {
+    DeviceGuard _dev(c);
     if (!c) return DWF_EINVAL;
     c->stream = (cudaStream_t)s;
     return DWF_OK;
 }
 
 dwf_status dwf_set_gauge(dwf_ctx* c, const void* U) {
+    DeviceGuard _dev(c);
     if (!c || !U) return DWF_EINVAL;
     const Geom& g = c->g;
     const int ng = c->compress12 ? 12 : 18;
@@ -483,6 +641,7 @@ dwf_status dwf_set_gauge(dwf_ctx* c, const void* U) {
     }
     c->wbytes64 = b64;
     c->wbytes32 = b32;
+    DWF_TRY(ws_alloc_all(c));
     DWF_TRY(launch_gauge_prep(c, (const double*)U));
     DWF_TRY(pipe_tables_upload(c));
     DWF_TRY(tma_state_build(c));
@@ -491,24 +650,29 @@ dwf_status dwf_set_gauge(dwf_ctx* c, const void* U) {
 }
 
 size_t dwf_field_bytes(const dwf_ctx* c, dwf_prec prec, dwf_parity parity) {
+    DeviceGuard _dev(c);
     if (!c) return 0;
     return half_bytes(c->g, prec) * (parity == DWF_FULL ? 2 : 1);
 }
 
 dwf_status dwf_pack(dwf_ctx* c, void* native, const void* canon, dwf_prec prec, dwf_parity parity) {
+    DeviceGuard _dev(c);
     if (!c || !native || !canon) return DWF_EINVAL;
     return launch_pack(c, native, canon, prec, parity, false);
 }
 dwf_status dwf_unpack(dwf_ctx* c, void* canon, const void* native, dwf_prec prec, dwf_parity parity) {
+    DeviceGuard _dev(c);
     if (!c || !native || !canon) return DWF_EINVAL;
     return launch_pack(c, const_cast<void*>(native), canon, prec, parity, true);
 }
 dwf_status dwf_convert(dwf_ctx* c, void* dst, dwf_prec dp, const void* src, dwf_prec sp, dwf_parity parity) {
+    DeviceGuard _dev(c);
     if (!c || !dst || !src || dst == src) return DWF_EINVAL;
     return launch_convert(c, dst, dp, src, sp, parity == DWF_FULL ? 2 : 1);
 }
 
 dwf_status dwf_dhop(dwf_ctx* c, void* out, const void* in, dwf_parity out_parity, int dagger, dwf_prec prec) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     if (!out || !in || out == in) { c->err = "dhop: null or aliased pointers"; return DWF_EINVAL; }
     if (out_parity == DWF_FULL) {
@@ -528,32 +692,39 @@ static dwf_status op5_public(dwf_ctx* c, void* out, const void* in, dwf_parity p
     return DWF_OK;
 }
 dwf_status dwf_meooe5d(dwf_ctx* c, void* out, const void* in, dwf_parity par, int dagger, dwf_prec prec) {
+    DeviceGuard _dev(c);
     return op5_public(c, out, in, par, dagger ? OP_ADAG : OP_A, prec);
 }
 dwf_status dwf_mooee(dwf_ctx* c, void* out, const void* in, dwf_parity par, int dagger, dwf_prec prec) {
+    DeviceGuard _dev(c);
     return op5_public(c, out, in, par, dagger ? OP_MEEDAG : OP_MEE, prec);
 }
 dwf_status dwf_mooee_inv(dwf_ctx* c, void* out, const void* in, dwf_parity par, int dagger, dwf_prec prec) {
+    DeviceGuard _dev(c);
     return op5_public(c, out, in, par, dagger ? OP_MEEINVDAG : OP_MEEINV, prec);
 }
 
 dwf_status dwf_m(dwf_ctx* c, void* out, const void* in, int dagger, dwf_prec prec) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     if (!out || !in || out == in) { c->err = "m: null or aliased pointers"; return DWF_EINVAL; }
     return m_apply(c, out, in, dagger, prec);
 }
 dwf_status dwf_mpc(dwf_ctx* c, void* out, const void* in, int dagger, dwf_prec prec) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     if (!out || !in || out == in) { c->err = "mpc: null or aliased pointers"; return DWF_EINVAL; }
     return mpc_apply(c, out, in, dagger, prec, -1);
 }
 dwf_status dwf_mdagm(dwf_ctx* c, void* out, const void* in, dwf_prec prec) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     if (!out || !in || out == in) { c->err = "mdagm: null or aliased pointers"; return DWF_EINVAL; }
     return mdagm_apply(c, out, in, prec);
 }
 
 dwf_status dwf_norm2(dwf_ctx* c, const void* v, dwf_prec prec, dwf_parity parity, double* result) {
+    DeviceGuard _dev(c);
     if (!c || !v || !result) return DWF_EINVAL;
     const size_t n = half_reals(c) * (parity == DWF_FULL ? 2 : 1);
     DWF_TRY(launch_norm2(c, v, prec, n, SLOT_T0));
@@ -562,6 +733,7 @@ dwf_status dwf_norm2(dwf_ctx* c, const void* v, dwf_prec prec, dwf_parity parity
 
 dwf_status dwf_cg(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, dwf_cg_mode mode, int use_guess,
                   dwf_cg_info* info) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     dwf_cg_info local;
     if (!info) info = &local;
@@ -578,8 +750,108 @@ dwf_status dwf_cg(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, 
     return st;
 }
 
+// ---- batched (multi right-hand side) fields and operators --------------------------------------
+namespace {
+struct BatchGuard {       // the batch count is only ever visible inside one ABI call
+    dwf_ctx* c;
+    BatchGuard(dwf_ctx* cc, int n) : c(cc) { c->nrhs_cur = n; }
+    ~BatchGuard() { c->nrhs_cur = 1; }
+};
+dwf_status mrhs_ok(dwf_ctx* c, int nrhs) {
+    if (nrhs < 1 || nrhs > MAXR) { c->err = "mrhs: nrhs must be 1..16"; return DWF_EINVAL; }
+    if ((long long)c->g.Vh * c->g.Ls * 12 * nrhs >= (1LL << 31)) { c->err = "mrhs: batched field too large for 32-bit vector indices"; return DWF_EINVAL; }
+    return DWF_OK;
+}
+}  // namespace
+
+dwf_status dwf_mrhs_reserve(dwf_ctx* c, int nrhs) {
+    DeviceGuard _dev(c);
+    if (!c) return DWF_EINVAL;
+    DWF_TRY(mrhs_ok(c, nrhs));
+    return nrhs > 1 ? wsm_reserve(c, nrhs) : DWF_OK;
+}
+
+size_t dwf_mrhs_field_bytes(const dwf_ctx* c, int nrhs, dwf_prec prec) {
+    if (!c || nrhs < 1) return 0;
+    return half_bytes(c->g, prec) * nrhs;
+}
+
+// strided copies between system j of a batched half field and a single native half field (tile by tile)
+dwf_status dwf_mrhs_insert(dwf_ctx* c, void* batched, int nrhs, int j, const void* single, dwf_prec prec) {
+    DeviceGuard _dev(c);
+    if (!c || !batched || !single) return DWF_EINVAL;
+    DWF_TRY(mrhs_ok(c, nrhs));
+    if (j < 0 || j >= nrhs) { c->err = "mrhs: system index out of range"; return DWF_EINVAL; }
+    const size_t chunk = half_bytes(c->g, prec) / c->g.ntiles;        // bytes of one tile of one system
+    DWF_CUDA_CHECK(c, cudaMemcpy2DAsync((char*)batched + j * chunk, chunk * nrhs, single, chunk, chunk, c->g.ntiles,
+                                        cudaMemcpyDeviceToDevice, c->stream));
+    return DWF_OK;
+}
+dwf_status dwf_mrhs_extract(dwf_ctx* c, void* single, const void* batched, int nrhs, int j, dwf_prec prec) {
+    DeviceGuard _dev(c);
+    if (!c || !batched || !single) return DWF_EINVAL;
+    DWF_TRY(mrhs_ok(c, nrhs));
+    if (j < 0 || j >= nrhs) { c->err = "mrhs: system index out of range"; return DWF_EINVAL; }
+    const size_t chunk = half_bytes(c->g, prec) / c->g.ntiles;
+    DWF_CUDA_CHECK(c, cudaMemcpy2DAsync(single, chunk, (const char*)batched + j * chunk, chunk * nrhs, chunk, c->g.ntiles,
+                                        cudaMemcpyDeviceToDevice, c->stream));
+    return DWF_OK;
+}
+
+dwf_status dwf_dhop_mrhs(dwf_ctx* c, void* out, const void* in, int nrhs, dwf_parity out_parity, int dagger, dwf_prec prec) {
+    DeviceGuard _dev(c);
+    DWF_TRY(need_gauge(c));
+    if (!out || !in || out == in || out_parity == DWF_FULL) { c->err = "dhop_mrhs: null / aliased pointers or FULL parity"; return DWF_EINVAL; }
+    DWF_TRY(mrhs_ok(c, nrhs));
+    BatchGuard bg(c, nrhs);
+    return launch_dhop(c, out, in, out_parity, dagger, prec);
+}
+
+dwf_status dwf_mpc_mrhs(dwf_ctx* c, void* out, const void* in, int nrhs, int dagger, dwf_prec prec) {
+    DeviceGuard _dev(c);
+    DWF_TRY(need_gauge(c));
+    if (!out || !in || out == in) { c->err = "mpc_mrhs: null or aliased pointers"; return DWF_EINVAL; }
+    DWF_TRY(mrhs_ok(c, nrhs));
+    if (nrhs > 1) DWF_TRY(wsm_reserve(c, nrhs));
+    BatchGuard bg(c, nrhs);
+    return mpc_apply(c, out, in, dagger, prec, -1);
+}
+
+dwf_status dwf_mdagm_mrhs(dwf_ctx* c, void* out, const void* in, int nrhs, dwf_prec prec) {
+    DeviceGuard _dev(c);
+    DWF_TRY(need_gauge(c));
+    if (!out || !in || out == in) { c->err = "mdagm_mrhs: null or aliased pointers"; return DWF_EINVAL; }
+    DWF_TRY(mrhs_ok(c, nrhs));
+    if (nrhs > 1) DWF_TRY(wsm_reserve(c, nrhs));
+    BatchGuard bg(c, nrhs);
+    return mdagm_apply(c, out, in, prec);
+}
+
+dwf_status dwf_cg_mrhs(dwf_ctx* c, void* x, const void* b, int nrhs, double tol, int max_iter, dwf_cg_mode mode, int use_guess,
+                       dwf_cg_info* info) {
+    DeviceGuard _dev(c);
+    DWF_TRY(need_gauge(c));
+    if (!x || !b || x == b || !info || tol <= 0.0 || max_iter < 0) { c->err = "cg_mrhs: bad arguments"; return DWF_EINVAL; }
+    DWF_TRY(mrhs_ok(c, nrhs));
+    memset(info, 0, sizeof(*info) * nrhs);
+    if (nrhs > 1) DWF_TRY(wsm_reserve(c, nrhs));
+    BatchGuard bg(c, nrhs);
+    const long long l0 = c->launches;
+    const double t0 = now_s();
+    dwf_status st = (mode == DWF_CG_MIXED) ? cg_mixed(c, x, b, tol, max_iter, use_guess, info)
+                                           : cg_f64(c, x, b, tol, max_iter, use_guess, info);
+    cudaStreamSynchronize(c->stream);
+    for (int j = 0; j < nrhs; ++j) {
+        info[j].seconds = now_s() - t0;
+        info[j].launches = (int)(c->launches - l0);
+    }
+    if (st == DWF_ENOTCONV) c->err = "cg_mrhs: max_iter reached";
+    return st;
+}
+
 dwf_status dwf_multishift_cg(dwf_ctx* c, void* xv, const void* b, const double* shifts, int nshift, double tol, int max_iter,
                              dwf_cg_info* info, double* resid_true) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     dwf_cg_info local;
     if (!info) info = &local;
@@ -672,6 +944,7 @@ dwf_status dwf_multishift_cg(dwf_ctx* c, void* xv, const void* b, const double* 
 }
 
 dwf_status dwf_chebyshev(dwf_ctx* c, void* out, const void* in, double lo, double hi, int order, dwf_prec prec) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     if (!out || !in || out == in || !(hi > lo) || order < 0) { c->err = "chebyshev: bad arguments"; return DWF_EINVAL; }
     const size_t hb = half_bytes(c->g, prec), n = half_reals(c);
@@ -702,6 +975,7 @@ dwf_status dwf_chebyshev(dwf_ctx* c, void* out, const void* in, double lo, doubl
 }
 
 dwf_status dwf_solve(dwf_ctx* c, void* psi, const void* eta, double tol, int max_iter, dwf_cg_mode mode, dwf_cg_info* info) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     dwf_cg_info local;
     if (!info) info = &local;
@@ -771,6 +1045,7 @@ static dwf_status boundary_geometry_ok(dwf_ctx* c) {
 }
 
 dwf_status dwf_domain_project(dwf_ctx* c, void* out, const void* in, int which, dwf_prec prec) {
+    DeviceGuard _dev(c);
     if (!c || !out || !in || which < 0 || which > 2) return DWF_EINVAL;
     DWF_TRY(boundary_geometry_ok(c));
     const size_t hb = half_bytes(c->g, prec);
@@ -796,6 +1071,7 @@ dwf_status boundary_block(dwf_ctx* c, void* out, const void* in, void* tmp, int 
 
 dwf_status dwf_boundary_op(dwf_ctx* c, void* out, const void* in, int inverse, double tol, int max_iter, dwf_cg_mode mode,
                            dwf_cg_info* info) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     dwf_cg_info local;
     if (!info) info = &local;
@@ -849,6 +1125,7 @@ dwf_status dwf_boundary_op(dwf_ctx* c, void* out, const void* in, int inverse, d
 }
 
 dwf_status dwf_dhop_host(dwf_ctx* c, void* out_host, const void* in_host, dwf_parity out_parity, int dagger, dwf_prec prec) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     if (!out_host || !in_host) return DWF_EINVAL;
     const size_t nb = dwf_field_bytes(c, prec, out_parity);
@@ -868,6 +1145,7 @@ dwf_status dwf_dhop_host(dwf_ctx* c, void* out_host, const void* in_host, dwf_pa
 }
 
 dwf_status dwf_mdagm_host(dwf_ctx* c, void* out_host, const void* in_host, dwf_prec prec) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     if (!out_host || !in_host) return DWF_EINVAL;
     const size_t nb = dwf_field_bytes(c, prec, DWF_ODD);
@@ -887,6 +1165,7 @@ dwf_status dwf_mdagm_host(dwf_ctx* c, void* out_host, const void* in_host, dwf_p
 
 dwf_status dwf_cg_host(dwf_ctx* c, void* x_host, const void* b_host, double tol, int max_iter, dwf_cg_mode mode,
                        dwf_cg_info* info) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     if (!x_host || !b_host) return DWF_EINVAL;
     const double t0 = now_s();
@@ -910,6 +1189,7 @@ dwf_status dwf_cg_host(dwf_ctx* c, void* x_host, const void* b_host, double tol,
 
 dwf_status dwf_solve_host(dwf_ctx* c, void* psi_host, const void* eta_host, double tol, int max_iter, dwf_cg_mode mode,
                           dwf_cg_info* info) {
+    DeviceGuard _dev(c);
     DWF_TRY(need_gauge(c));
     if (!psi_host || !eta_host) return DWF_EINVAL;
     const double t0 = now_s();

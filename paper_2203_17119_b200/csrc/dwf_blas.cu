@@ -7,8 +7,14 @@
 
 namespace dwf {
 
-dwf_status ensure_partials(dwf_ctx* c, int n);
-dwf_status launch_reduce(dwf_ctx* c, int n, int slot);
+// Batched fields (dwf_internal.h): the kernels that need a per-system scalar run with blockIdx.y = right-hand side and map
+// their running index i over ONE system's vectors to the batched field: i = tile * chunk + off -> (tile * N + rhs) * chunk + off,
+// chunk = Ls * K * TS vectors (one tile of one system).  N = 1: the identity.
+__device__ __forceinline__ size_t rhs_index(size_t i, unsigned chunk) {
+    if (gridDim.y == 1) return i;
+    const size_t tile = i / chunk;
+    return (tile * gridDim.y + blockIdx.y) * chunk + (i - tile * chunk);
+}
 
 template <typename R> struct VB;
 template <> struct VB<float> { using V = float4; static constexpr int VW = 4; };
@@ -42,41 +48,48 @@ __device__ __forceinline__ double2 axpyv(double a, const double2& x, const doubl
 }
 
 template <typename R>
-__global__ void __launch_bounds__(256) norm2_kernel(const typename VB<R>::V* __restrict__ v, size_t nvec,
+__global__ void __launch_bounds__(256) norm2_kernel(const typename VB<R>::V* __restrict__ v, size_t nvec, unsigned chunk,
                                                     double* __restrict__ partials) {
     double acc = 0.0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x)
-        acc += n2(v[i]);
+        acc += n2(v[rhs_index(i, chunk)]);
     double tot = blk_sum(acc);
-    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+    if (threadIdx.x == 0) partials[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = tot;
 }
 
 // x += a p ; r -= a z ; partial |r|^2 ;  a = sc[slot_c]/sc[slot_d]
 template <typename R>
 __global__ void __launch_bounds__(256) cg_update_kernel(typename VB<R>::V* __restrict__ x, typename VB<R>::V* __restrict__ r,
                                                         const typename VB<R>::V* __restrict__ p,
-                                                        const typename VB<R>::V* __restrict__ z, size_t nvec,
+                                                        const typename VB<R>::V* __restrict__ z, size_t nvec, unsigned chunk,
                                                         const double* __restrict__ sc, int slot_c, int slot_d,
-                                                        double* __restrict__ partials) {
-    const R a = (R)(sc[slot_c] / sc[slot_d]);
+                                                        double* __restrict__ partials, const int* __restrict__ conv, int iter) {
+    const int rhs = blockIdx.y;
+    const R a = (R)(sc[slot_c * MAXR + rhs] / sc[slot_d * MAXR + rhs]);
+    const int cv = conv[rhs];
+    const bool frozen = (cv >= 0 && cv < iter);       // stopping test fired at an earlier iteration: x stays
     double acc = 0.0;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
-        x[i] = axpyv(a, p[i], x[i]);
+    for (size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i0 < nvec; i0 += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = rhs_index(i0, chunk);
+        if (!frozen) x[i] = axpyv(a, p[i], x[i]);
         typename VB<R>::V rn = axpyv(-a, z[i], r[i]);
         r[i] = rn;
         acc += n2(rn);
     }
     double tot = blk_sum(acc);
-    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+    if (threadIdx.x == 0) partials[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = tot;
 }
 
 // p = r + b p ; b = sc[slot_cn]/sc[slot_c]
 template <typename R>
 __global__ void __launch_bounds__(256) xpay_kernel(typename VB<R>::V* __restrict__ p, const typename VB<R>::V* __restrict__ r,
-                                                   size_t nvec, const double* __restrict__ sc, int slot_cn, int slot_c) {
-    const R b = (R)(sc[slot_cn] / sc[slot_c]);
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x)
+                                                   size_t nvec, unsigned chunk, const double* __restrict__ sc, int slot_cn,
+                                                   int slot_c) {
+    const R b = (R)(sc[slot_cn * MAXR + blockIdx.y] / sc[slot_c * MAXR + blockIdx.y]);
+    for (size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i0 < nvec; i0 += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = rhs_index(i0, chunk);
         p[i] = axpyv(b, p[i], r[i]);
+    }
 }
 
 // y += a x
@@ -161,51 +174,61 @@ static inline int blas_grid(size_t nvec) {
 #define DWF_BLAS_DISPATCH(prec, CALL32, CALL64) \
     do { if ((prec) == DWF_F64) { CALL64; } else { CALL32; } } while (0)
 
+// vectors of one tile of one system (the unit the batched layout interleaves)
+static inline unsigned tile_chunk(const dwf_ctx* c, int prec) { return (unsigned)c->g.Ls * (prec == DWF_F64 ? 12 : 6) * c->g.TS; }
+
+// nreal: reals of ONE system; with c->nrhs_cur > 1 the field is batched and every system gets its own norm
 dwf_status launch_norm2(dwf_ctx* c, const void* v, int prec, size_t nreal, int slot) {
     const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
-    const int grid = blas_grid(nvec);
-    dwf_status st = ensure_partials(c, grid);
+    const int gridx = blas_grid(nvec);
+    const dim3 grid(gridx, c->nrhs_cur);
+    const unsigned chunk = tile_chunk(c, prec);
+    dwf_status st = ensure_partials(c, gridx);
     if (st != DWF_OK) return st;
-    DWF_BLAS_DISPATCH(prec, (norm2_kernel<float><<<grid, 256, 0, c->stream>>>((const float4*)v, nvec, c->partials)),
-                      (norm2_kernel<double><<<grid, 256, 0, c->stream>>>((const double2*)v, nvec, c->partials)));
+    DWF_BLAS_DISPATCH(prec, (norm2_kernel<float><<<grid, 256, 0, c->stream>>>((const float4*)v, nvec, chunk, c->partials)),
+                      (norm2_kernel<double><<<grid, 256, 0, c->stream>>>((const double2*)v, nvec, chunk, c->partials)));
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
-    return launch_reduce(c, grid, slot);
+    return launch_reduce(c, gridx, slot);
 }
 
 dwf_status launch_cg_update(dwf_ctx* c, void* x, void* r, const void* p, const void* z, int prec, size_t nreal,
-                            int slot_c, int slot_d, int slot_cn) {
+                            int slot_c, int slot_d, int slot_cn, int iter) {
     const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
-    const int grid = blas_grid(nvec);
-    dwf_status st = ensure_partials(c, grid);
+    const int gridx = blas_grid(nvec);
+    const dim3 grid(gridx, c->nrhs_cur);
+    const unsigned chunk = tile_chunk(c, prec);
+    dwf_status st = ensure_partials(c, gridx);
     if (st != DWF_OK) return st;
     DWF_BLAS_DISPATCH(prec,
                       (cg_update_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)x, (float4*)r, (const float4*)p,
-                                                                          (const float4*)z, nvec, c->scalars, slot_c,
-                                                                          slot_d, c->partials)),
+                                                                          (const float4*)z, nvec, chunk, c->scalars, slot_c,
+                                                                          slot_d, c->partials, c->cg_conv, iter)),
                       (cg_update_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)x, (double2*)r, (const double2*)p,
-                                                                           (const double2*)z, nvec, c->scalars, slot_c,
-                                                                           slot_d, c->partials)));
+                                                                           (const double2*)z, nvec, chunk, c->scalars, slot_c,
+                                                                           slot_d, c->partials, c->cg_conv, iter)));
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
-    return launch_reduce(c, grid, slot_cn);
+    return launch_reduce(c, gridx, slot_cn, iter);
 }
 
 dwf_status launch_xpay(dwf_ctx* c, void* p, const void* r, int prec, size_t nreal, int slot_cn, int slot_c) {
     const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
-    const int grid = blas_grid(nvec);
+    const dim3 grid(blas_grid(nvec), c->nrhs_cur);
+    const unsigned chunk = tile_chunk(c, prec);
     DWF_BLAS_DISPATCH(prec,
-                      (xpay_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)p, (const float4*)r, nvec, c->scalars,
+                      (xpay_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)p, (const float4*)r, nvec, chunk, c->scalars,
                                                                      slot_cn, slot_c)),
-                      (xpay_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)p, (const double2*)r, nvec, c->scalars,
+                      (xpay_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)p, (const double2*)r, nvec, chunk, c->scalars,
                                                                       slot_cn, slot_c)));
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
     return DWF_OK;
 }
 
+// elementwise kernels: nreal reals per system, all c->nrhs_cur systems of a batched field at once
 dwf_status launch_axpy(dwf_ctx* c, void* y, const void* x, double a, int prec, size_t nreal) {
-    const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
+    const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4) * c->nrhs_cur;
     const int grid = blas_grid(nvec);
     DWF_BLAS_DISPATCH(prec, (axpy_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)y, (const float4*)x, (float)a, nvec)),
                       (axpy_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)y, (const double2*)x, a, nvec)));
@@ -215,7 +238,7 @@ dwf_status launch_axpy(dwf_ctx* c, void* y, const void* x, double a, int prec, s
 }
 
 dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int prec, size_t nreal) {
-    const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
+    const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4) * c->nrhs_cur;
     const int grid = blas_grid(nvec);
     DWF_BLAS_DISPATCH(prec,
                       (sub_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)out, (const float4*)a, (const float4*)b, nvec)),

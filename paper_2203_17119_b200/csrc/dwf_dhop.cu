@@ -106,7 +106,7 @@ __global__ void __launch_bounds__(256) dhop_kernel(Geom g, const typename VT<R>:
 template <typename R, int SC, int NG>
 static dwf_status launch_t(dwf_ctx* c, void* out, const void* in, const void* W, int out_parity, int dagger) {
     using V = typename VT<R>::V;
-    const Geom g = geom_prec(c, sizeof(R) == 8 ? DWF_F64 : DWF_F32);
+    const Geom g = geom_prec(c, sizeof(R) == 8 ? DWF_F64 : DWF_F32, c->nrhs_cur);
     const int nchunks = (g.Ls + SC - 1) / SC;
     int block = 128;
     if (g.TS < block) block = ((g.TS + 31) / 32) * 32;
@@ -177,7 +177,8 @@ dwf_status launch_dhop(dwf_ctx* c, void* out, const void* in, int out_parity, in
     st = launch_dhop_untimed(c, out, in, out_parity, dagger, prec);
     if (st != DWF_OK) return st;
     const double B = (prec == DWF_F64) ? 8.0 : 4.0;
-    return dhop_time_end(c, 2.0 * half_bytes(c->g, prec) + (double)c->g.Vh * 8 * (c->compress12 ? 12 : 18) * B);
+    // algorithmic bytes: every system's field in and out, the links once for all of them
+    return dhop_time_end(c, 2.0 * half_bytes(c->g, prec) * c->nrhs_cur + (double)c->g.Vh * 8 * (c->compress12 ? 12 : 18) * B);
 }
 
 static dwf_status launch_dhop_untimed(dwf_ctx* c, void* out, const void* in, int out_parity, int dagger, int prec) {

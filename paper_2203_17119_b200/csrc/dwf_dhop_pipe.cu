@@ -325,11 +325,9 @@ static dwf_status launch_pipe_t(dwf_ctx* c, const PipeArgs& a) {
     constexpr int K = VT<R>::K;
     const size_t smem = (size_t)NST * K * NSLOT * sizeof(V);
     auto kern = dhop_pipe_kernel<R, TPS, NG, TS, NSLOT, NST>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    static unsigned long long attr_done = 0;      // per device (dwf_internal.h)
+    if (attr_needed(attr_done, c->device))
         DWF_CUDA_CHECK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
     kern<<<c->g.ntiles, TS * TPS, smem, c->stream>>>(a);
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
@@ -346,7 +344,7 @@ dwf_status launch_dhop_pipe(dwf_ctx* c, void* out, const void* in, int out_parit
     *handled = false;
     const int pr = (prec == DWF_F64) ? 1 : 0;
     if (!c->pipe_nbslot[pr] || c->g.Ls < 1) return DWF_OK;
-    const Geom g = geom_prec(c, prec);
+    const Geom g = geom_prec(c, prec, c->nrhs_cur);
     PipeArgs a;
     a.g = g; a.in = in; a.out = out;
     a.W = (prec == DWF_F64) ? c->W64[out_parity] : c->W32[out_parity];

@@ -210,22 +210,33 @@ std::vector<uint32_t> build_order(const Geom& g, int code, int axes_code) {
     std::vector<uint32_t> o;
     o.reserve(g.ntiles);
     const int nblobs = NB[0] * NB[1] * NB[2] * NB[3];
-    for (int ib = 0; ib < nblobs; ++ib) {
+    auto blob_coords = [&](int ib, int bc[4]) {
         // mixed-radix digits of ib (ax[0] fastest), reflected when the sum of the higher digits is odd
         int d[4], r = ib;
         for (int i = 0; i < 4; ++i) { d[i] = r % NB[ax[i]]; r /= NB[ax[i]]; }
-        int bc[4];
         for (int i = 3; i >= 0; --i) {
             int hi = 0;
             for (int j = i + 1; j < 4; ++j) hi += d[j];
             bc[ax[i]] = (hi & 1) ? NB[ax[i]] - 1 - d[i] : d[i];
+        }
+    };
+    for (int ib = 0; ib < nblobs; ++ib) {
+        int bc[4];
+        blob_coords(ib, bc);
+        // t-sweep direction of this blob (bits 30-31 of its entries: 1 = the next blob is the +t neighbour, 2 = the -t one, 0 = neither):
+        // tells the producer which t-slabs the NEXT round will read again (L2 retention hints)
+        uint32_t dirflag = 0;
+        if (B[3] == 1 && ib + 1 < nblobs) {
+            int nb[4];
+            blob_coords(ib + 1, nb);
+            if (nb[0] == bc[0] && nb[1] == bc[1] && nb[2] == bc[2]) dirflag = (nb[3] == bc[3] + 1) ? 1u : (nb[3] == bc[3] - 1 ? 2u : 0u);
         }
         for (int t = 0; t < B[3]; ++t)
             for (int z = 0; z < B[2]; ++z)
                 for (int y = 0; y < B[1]; ++y)
                     for (int x = 0; x < B[0]; ++x) {
                         const int c[4] = {bc[0] * B[0] + x, bc[1] * B[1] + y, bc[2] * B[2] + z, bc[3] * B[3] + t};
-                        o.push_back((uint32_t)tile_index(g, c));
+                        o.push_back((uint32_t)tile_index(g, c) | (dirflag << 30));
                     }
     }
     return o;
@@ -262,7 +273,7 @@ struct TmaState {
     int* counters = nullptr;      // device [3]: next position in `order`, CTAs done, round arrivals (self-resetting, see the kernel)
     int K_built = 0;
     int num_sms = 0;
-    struct Maps { const void* ptr; int prec; CUtensorMap m[3]; };
+    struct Maps { const void* ptr; int prec; int Ls; CUtensorMap m[3]; };
     std::vector<Maps> cache;      // small LRU of tensor maps per input pointer
 };
 
@@ -290,9 +301,7 @@ dwf_status tma_state_build(dwf_ctx* c) {
     if (!encode_fn()) return DWF_OK;
     TmaState* s = new TmaState();
     c->tma = s;
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, dev);
+    cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, c->device);
     // fp64 tables first (K = 12, XOR-rotated lane order), fp32 second (K = 6, plain order)
     TmaTables t64 = build_tma_tables_swz(12), t32 = build_tma_tables_plain(6);
     std::vector<uint16_t> off(t64.off);
@@ -320,8 +329,9 @@ dwf_status tma_state_build(dwf_ctx* c) {
 // [2] y faces (32-byte rows).  A native half field is nrows = ntiles*Ls*K rows of 2048 bytes (one (tile,s,k) each).
 static dwf_status get_maps(dwf_ctx* c, const void* in, int prec, const CUtensorMap** out) {
     TmaState* s = (TmaState*)c->tma;
+    const int LsT = c->g.Ls * c->nrhs_cur;                // batched fields: one long fifth dimension
     for (size_t i = 0; i < s->cache.size(); ++i)
-        if (s->cache[i].ptr == in && s->cache[i].prec == prec) {
+        if (s->cache[i].ptr == in && s->cache[i].prec == prec && s->cache[i].Ls == LsT) {
             if (i != 0) std::swap(s->cache[i], s->cache[0]);
             *out = s->cache[0].m;
             return DWF_OK;
@@ -329,10 +339,10 @@ static dwf_status get_maps(dwf_ctx* c, const void* in, int prec, const CUtensorM
     const Geom& g = c->g;
     const int K = (prec == DWF_F64) ? 12 : 6;
     const int epv = (prec == DWF_F64) ? 2 : 4;             // elements per 16-byte vector
-    const cuuint64_t nrows = (cuuint64_t)g.ntiles * g.Ls * K;
+    const cuuint64_t nrows = (cuuint64_t)g.ntiles * LsT * K;
     const CUtensorMapDataType dt = (prec == DWF_F64) ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
     TmaState::Maps m;
-    m.ptr = in; m.prec = prec;
+    m.ptr = in; m.prec = prec; m.Ls = LsT;
     EncodeTiledFn enc = encode_fn();
     const cuuint32_t ones[4] = {1, 1, 1, 1};
     CUresult r;
@@ -397,6 +407,23 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
 __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, uint32_t bar) {
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
                  ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_3d_hint(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar, uint64_t pol) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;"
+                 ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ uint64_t policy_evict_last() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ uint64_t policy_evict_first() {
+    uint64_t p;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+    return p;
+}
+__device__ __forceinline__ void l2_prefetch_bulk_hint(const void* p, uint32_t bytes, uint64_t pol) {
+    asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(p), "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void l2_prefetch(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
@@ -480,8 +507,9 @@ __device__ __forceinline__ void recon_s(const R (&g)[12], R s, R (&acc)[24]) {
 struct EpiArgs {
     int mode;              // EPI_NONE or EPI_FINAL
     const void* xin;       // the field Mee acts on (output parity)
-    double* partials;      // per-CTA partial sums of |out|^2; null: none
+    double* partials;      // partial sums of |out|^2, one per (system, tile): partials[rhs * ntiles + tile]; null: none
     double bee, mcee, mf, scale;     // Mee = bee + mcee Q
+    int Ls0;               // physical Ls: a batched field has g.Ls = N * Ls0 slices per tile, walls at s mod Ls0 = 0, Ls0 - 1
 };
 
 __device__ __forceinline__ float4 vmul(float a, const float4& x) { return make_float4(a * x.x, a * x.y, a * x.z, a * x.w); }
@@ -499,6 +527,14 @@ __device__ __forceinline__ double vnorm2(const double2& a) { return a.x * a.x + 
 __device__ __forceinline__ float4 ldcs_v(const float4* p) { return __ldcs(p); }
 __device__ __forceinline__ double2 ldcs_v(const double2* p) { return __ldcs(p); }
 
+// halo regions the producer does not load: a traffic-attribution aid of the probe build only (results are then wrong);
+// the product build compiles every test on it away
+#ifdef DWF_PROBE
+#define SKIPM (a.skip)
+#else
+#define SKIPM 0
+#endif
+
 struct TmaArgs {
     Geom g;
     const void* in;
@@ -512,6 +548,7 @@ struct TmaArgs {
     const uint32_t* order;    // [ntiles]
     int* counters;            // [3] queue / done / round-arrival counters
     EpiArgs epi;
+    int l2hint;               // bit 0: t-slab retention hints along the sweep, bit 1: links prefetched evict_first
     int skip;                 // debug: bit r set = do not load halo region r (4..11); results are then wrong, traffic only
     int mode;                 // 0: static round-robin, 1: global in-order queue
     int dagger;
@@ -585,8 +622,10 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                 if (lane == 0) v = atomicAdd(a.counters, 1) + (int)gridDim.x;
                 it_next = __shfl_sync(0xffffffffu, v, 0);
             }
-            const int tile = a.order[it];
-            const int tile_next = (it_next < ntiles) ? (int)a.order[it_next] : -1;
+            const uint32_t oent = a.order[it];
+            const int tile = (int)(oent & 0x3fffffffu);
+            const int tdir = (a.l2hint & 1) ? (int)(oent >> 30) : 0;      // 1: the next round reads the +t neighbours, 2: the -t ones
+            const int tile_next = (it_next < ntiles) ? (int)(a.order[it_next] & 0x3fffffffu) : -1;
             int tc[4];
             tile_coords(g, tile, tc);
             int nt[8];
@@ -611,30 +650,46 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                 if (lane == 0) {
                     // next tile's links -> L2, issued with this tile's last slice: the consumers want them NST slices
                     // later (issued a whole tile ahead they were evicted again before use and fetched twice)
-                    if (s == Ls - 1 && tile_next >= 0)
-                        l2_prefetch_bulk(reinterpret_cast<const V*>(a.W) + (size_t)tile_next * 8 * KG * TSV, 8 * KG * TSV * 16);
-                    const int nskip = __popc(a.skip & (GATHER_Y ? 0x0f0 : 0x3f0));
+                    if (s == Ls - 1 && tile_next >= 0) {
+                        const V* wn = reinterpret_cast<const V*>(a.W) + (size_t)tile_next * 8 * KG * TSV;
+                        if (a.l2hint & 2) l2_prefetch_bulk_hint(wn, 8 * KG * TSV * 16, policy_evict_first());
+                        else l2_prefetch_bulk(wn, 8 * KG * TSV * 16);
+                    }
+                    const int nskip = __popc(SKIPM & (GATHER_Y ? 0x0f0 : 0x3f0));
                     mbar_arrive_expect_tx(full, (NTMA - nskip) * REGION_BYTES);
                     const int row_own = (tile * Ls + s) * K;
+                    if (tdir == 0) {
 #pragma unroll
-                    for (int tt = 0; tt < 4; ++tt) tma_load_3d(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full);
-                    if (!(a.skip & 0x010)) tma_load_3d(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full);
-                    if (!(a.skip & 0x020)) tma_load_3d(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full);
-                    if (!(a.skip & 0x040)) tma_load_4d(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full);
-                    if (!(a.skip & 0x080)) tma_load_4d(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full);
+                        for (int tt = 0; tt < 4; ++tt) tma_load_3d(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full);
+                        if (!(SKIPM & 0x010)) tma_load_3d(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full);
+                        if (!(SKIPM & 0x020)) tma_load_3d(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full);
+                    } else {
+                        // the t sweep reads two slabs of this working set again one round later (the leading own slab as the
+                        // next tile's trailing face, the leading face as its own slab): keep those in L2, drop the trailing ones
+                        const uint64_t keep = policy_evict_last(), drop = policy_evict_first();
+                        const bool up = (tdir == 1);
+                        tma_load_3d_hint(base + 0 * REGION_BYTES, &map_slab, 0, 0, row_own, full, up ? drop : keep);
+                        tma_load_3d(base + 1 * REGION_BYTES, &map_slab, 0, 1, row_own, full);
+                        tma_load_3d(base + 2 * REGION_BYTES, &map_slab, 0, 2, row_own, full);
+                        tma_load_3d_hint(base + 3 * REGION_BYTES, &map_slab, 0, 3, row_own, full, up ? keep : drop);
+                        if (!(SKIPM & 0x010)) tma_load_3d_hint(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full, up ? keep : drop);
+                        if (!(SKIPM & 0x020)) tma_load_3d_hint(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full, up ? drop : keep);
+                    }
+                    if (!(SKIPM & 0x040)) tma_load_4d(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full);
+                    if (!(SKIPM & 0x080)) tma_load_4d(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full);
                     if (!GATHER_Y) {
-                        if (!(a.skip & 0x100)) tma_load_4d(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full);
-                        if (!(a.skip & 0x200)) tma_load_4d(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full);
+                        if (!(SKIPM & 0x100)) tma_load_4d(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full);
+                        if (!(SKIPM & 0x200)) tma_load_4d(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full);
                     }
                 }
                 const V* src = in + (size_t)s * (K * TSV);
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-                    if (!(a.skip & 0x400)) cp_async16_tma(base + gd0 + k * 512, src + i0 + k * TSV);
-                    if (!(a.skip & 0x800)) cp_async16_tma(base + gd1 + k * 512, src + i1 + k * TSV);
+                    if (!(SKIPM & 0x400)) cp_async16_tma(base + gd0 + k * 512, src + i0 + k * TSV);
+                    if (!(SKIPM & 0x800)) cp_async16_tma(base + gd1 + k * 512, src + i1 + k * TSV);
                     if (GATHER_Y) {
-                        if (!(a.skip & 0x100)) cp_async16_tma(base + gd2 + k * 512, src + i2 + k * TSV);
-                        if (!(a.skip & 0x200)) cp_async16_tma(base + gd3 + k * 512, src + i3 + k * TSV);
+                        if (!(SKIPM & 0x100)) cp_async16_tma(base + gd2 + k * 512, src + i2 + k * TSV);
+                        if (!(SKIPM & 0x200)) cp_async16_tma(base + gd3 + k * 512, src + i3 + k * TSV);
                     }
                 }
                 cp_async_mbar_arrive_noinc(full);
@@ -668,9 +723,9 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
     }
     const int tt = site >> 5;
     const R dsgn = a.dagger ? (R)-1 : (R)1;
-    uint32_t n = 0, j = 0;
+    uint32_t n = 0, j = 0, nred = 0;
     double nrm = 0.0;
-    int tile = a.order[blockIdx.x];
+    int tile = (int)(a.order[blockIdx.x] & 0x3fffffffu);
     while (tile >= 0) {
         int tile_next = -1;
         const int tct = tile / (g.NT[0] * g.NT[1] * g.NT[2]);
@@ -696,23 +751,25 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
         }
         V* __restrict__ outp = reinterpret_cast<V*>(a.out) + (size_t)tile * Ls * K * TSV + site;
         const V* __restrict__ xin_t = reinterpret_cast<const V*>(a.epi.xin) + (size_t)tile * Ls * K * TSV + site;
+        // fused epilogue on a batched field: sl = slice within its system (0 .. Ls0-1), rb = first slice of that system
+        int sl = 0, rb = 0;
         for (int s = 0; s < Ls; ++s, ++n) {
             const uint32_t st = n % NST, ph = (n / NST) & 1;
             const uint32_t base = stage0 + st * STAGE_BYTES;
             mbar_wait(bar0 + 8 * st, ph);
             if (s == 0) tile_next = *(volatile int*)&next_of[j & 3];
             if constexpr (EPI != 0) {
-                // the epilogue's xin rows -> L2 one slice ahead (slice 0 also fetches itself and the wall slice)
+                // the epilogue's xin rows -> L2 one slice ahead (a system's slice 0 also fetches itself and the wall slice)
                 const V* xk = xin_t + ((TPS == 1) ? 0 : sub * (K / 2)) * TSV;
                 if (s + 1 < Ls) {
 #pragma unroll
                     for (int k = 0; k < 6; ++k) l2_prefetch(xk + (size_t)(s + 1) * (K * TSV) + k * TSV);
                 }
-                if (s == 0) {
+                if (sl == 0) {
 #pragma unroll
                     for (int k = 0; k < 6; ++k) {
-                        l2_prefetch(xk + k * TSV);
-                        l2_prefetch(xk + (size_t)(Ls - 1) * (K * TSV) + k * TSV);
+                        l2_prefetch(xk + (size_t)s * (K * TSV) + k * TSV);
+                        l2_prefetch(xk + (size_t)(rb + a.epi.Ls0 - 1) * (K * TSV) + k * TSV);
                     }
                 }
             }
@@ -737,11 +794,12 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
             V* o = outp + (size_t)s * (K * TSV);
             // EPI: out_s = bee xin_s + mcee (Q xin)_s + scale D_s, |out|^2 summed (Mee xin - 1/4 Dhop ..., reading C6)
             const R e_bee = (R)a.epi.bee, e_scale = (R)a.epi.scale;
-            const R e_wm = (R)((s > 0) ? a.epi.mcee : -a.epi.mf * a.epi.mcee);            // P+ : xin_{s-1}
-            const R e_wp = (R)((s + 1 < Ls) ? a.epi.mcee : -a.epi.mf * a.epi.mcee);       // P- : xin_{s+1}
+            const int Ls0 = (EPI != 0) ? a.epi.Ls0 : Ls;
+            const R e_wm = (R)((sl > 0) ? a.epi.mcee : -a.epi.mf * a.epi.mcee);            // P+ : xin_{s-1}
+            const R e_wp = (R)((sl + 1 < Ls0) ? a.epi.mcee : -a.epi.mf * a.epi.mcee);      // P- : xin_{s+1}
             const V* xs = xin_t + (size_t)s * (K * TSV);
-            const V* xm = xin_t + (size_t)((s > 0) ? s - 1 : Ls - 1) * (K * TSV);
-            const V* xp = xin_t + (size_t)((s + 1 < Ls) ? s + 1 : 0) * (K * TSV);
+            const V* xm = xin_t + (size_t)((sl > 0) ? s - 1 : rb + Ls0 - 1) * (K * TSV);
+            const V* xp = xin_t + (size_t)((sl + 1 < Ls0) ? s + 1 : rb) * (K * TSV);
             if (TPS == 1) {
                 if constexpr (EPI != 0) {
 #pragma unroll
@@ -782,22 +840,27 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                     for (int k = 0; k < K / 2; ++k) stcs_v(o2 + k * TSV, packv(mine + k * VW));
                 }
             }
-        }
-        if constexpr (EPI != 0) {
-            // |out|^2 of this tile: fixed-tree sum over the consumer threads into partials[tile] -- independent of which
-            // CTA took the tile, so the reduction is bit-reproducible under the dynamic tile queue as well
-            if (a.epi.partials != nullptr) {
+            if constexpr (EPI != 0) {
+                if (++sl == Ls0) {
+                    // |out|^2 of this (system, tile): fixed-tree sum over the consumer threads into partials[rhs][tile] --
+                    // independent of which CTA took the tile, so the reduction is bit-reproducible under the dynamic queue
+                    if (a.epi.partials != nullptr) {
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o);
-                if (lane == 0) wsum[j & 1][cw] = nrm;
-                asm volatile("bar.sync 1, %0;" ::"n"(128 * TPS) : "memory");
-                if (ctid == 0) {
-                    double t = 0.0;
+                        for (int o2 = 16; o2 > 0; o2 >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o2);
+                        if (lane == 0) wsum[nred & 1][cw] = nrm;
+                        asm volatile("bar.sync 1, %0;" ::"n"(128 * TPS) : "memory");
+                        if (ctid == 0) {
+                            double t = 0.0;
 #pragma unroll
-                    for (int i = 0; i < NCW; ++i) t += wsum[j & 1][i];
-                    a.epi.partials[tile] = t;
+                            for (int i = 0; i < NCW; ++i) t += wsum[nred & 1][i];
+                            a.epi.partials[(size_t)(rb / Ls0) * ntiles + tile] = t;
+                        }
+                        nrm = 0.0;
+                        ++nred;
+                    }
+                    sl = 0;
+                    rb = s + 1;
                 }
-                nrm = 0.0;
             }
         }
         tile = tile_next;
@@ -811,11 +874,9 @@ static dwf_status launch_tma_t(dwf_ctx* c, const TmaArgs& a, const CUtensorMap* 
     constexpr int K = VT<R>::K;
     const size_t smem = (size_t)NST * NREG * K * 512;
     auto kern = dhop_tma_kernel<R, TPS, NG, NST, MINB, EPI>;
-    static bool attr_done = false;
-    if (!attr_done) {
+    static unsigned long long attr_done = 0;      // per device (dwf_internal.h)
+    if (attr_needed(attr_done, c->device))
         DWF_CUDA_CHECK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        attr_done = true;
-    }
     TmaState* s = (TmaState*)c->tma;
     int grid = s->num_sms * MINB;
     if (c->dhop_grid > 0) grid = c->dhop_grid;
@@ -833,7 +894,7 @@ static dwf_status fill_args(dwf_ctx* c, TmaArgs& a, void* out, const void* in, i
     dwf_status st = get_maps(c, in, prec, maps);
     if (st != DWF_OK) return st;
     memset(&a, 0, sizeof(a));
-    a.g = geom_prec(c, prec); a.in = in; a.out = out;
+    a.g = geom_prec(c, prec, c->nrhs_cur); a.in = in; a.out = out;
     a.W = (prec == DWF_F64) ? c->W64[out_parity] : c->W32[out_parity];
     a.off = s->off + (size_t)(prec == DWF_F64 ? 0 : 2 * 8 * TSV) + (size_t)out_parity * 8 * TSV;
     a.gsrc = s->gsrc + (size_t)out_parity * 4 * 32;
@@ -843,7 +904,10 @@ static dwf_status fill_args(dwf_ctx* c, TmaArgs& a, void* out, const void* in, i
     a.order = s->order;
     a.counters = s->counters;
     a.mode = c->dhop_dynamic;
+#ifdef DWF_PROBE
     a.skip = c->dhop_skip;
+#endif
+    a.l2hint = c->dhop_l2hint;
     a.dagger = dagger;
     a.epi.mode = EPI_NONE;
     return DWF_OK;
@@ -880,6 +944,7 @@ dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_pari
     e.mode = EPI_FINAL;
     e.xin = xin;
     e.bee = bee; e.mcee = -cee; e.mf = c->mf; e.scale = scale;
+    e.Ls0 = c->g.Ls;
     int grid = 0;
     if (norm_slot >= 0) {
         st = ensure_partials(c, c->g.ntiles);              // one partial per tile
@@ -893,9 +958,9 @@ dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_pari
     if (st != DWF_OK) return st;
     // algorithmic bytes: the input field, xin, the links, one field written
     const double B = (prec == DWF_F64) ? 8.0 : 4.0;
-    st = dhop_time_end(c, 3.0 * (double)half_bytes(c->g, prec) + (double)c->g.Vh * 8 * 12 * B);
+    st = dhop_time_end(c, 3.0 * (double)half_bytes(c->g, prec) * c->nrhs_cur + (double)c->g.Vh * 8 * 12 * B);
     if (st != DWF_OK) return st;
-    if (norm_slot >= 0) return launch_reduce(c, c->g.ntiles, norm_slot);
+    if (norm_slot >= 0) return launch_reduce(c, c->g.ntiles, norm_slot, 0);
     return DWF_OK;
 }
 

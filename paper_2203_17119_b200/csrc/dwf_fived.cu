@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(128) op5_kernel(int Ls_rt, int TS, unsigned nv
         const unsigned tile = gid / per_tile, j = gid - tile * per_tile;
         const int k = j / TS;
         const int chir = (k < K / 2) ? 0 : 1;
-        const size_t base = (size_t)tile * Ls * per_tile + j;
+        const size_t base = ((size_t)tile * gridDim.y + blockIdx.y) * Ls * per_tile + j;     // blockIdx.y: right-hand side
         const R* t1 = sT1 + chir * Ls * Ls;
         const R* t2 = sT2 + chir * Ls * Ls;
         if (LS > 0) {
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(128) op5_kernel(int Ls_rt, int TS, unsigned nv
     }
     if (partials != nullptr) {
         double tot = block_reduce_sum(nrm);
-        if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+        if (threadIdx.x == 0) partials[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = tot;
     }
 }
 
@@ -183,27 +183,35 @@ __global__ void __launch_bounds__(128) op5_kernel(int Ls_rt, int TS, unsigned nv
 // CG vector step fused with the next A p (fused CG loop, dwf_api.cu):  x += alpha p;  p <- r + beta p;  ap = A p,
 // A = b5 + c5 Q (reading C5).  One thread owns one 16-byte vector column of one 4-D site and walks it in sweep order
 // (s ascending on P+ components, descending on P-), so (Q p)_j is the previous element, the -mf wall at j = 0.
-// init: p <- r, ap = A p, x untouched.  alpha = sc[slot_c]/sc[slot_d], beta = sc[slot_cn]/sc[slot_c].
+// init: p <- r, ap = A p, x untouched.  alpha = sc[slot_c]/sc[slot_d], beta = sc[slot_cn]/sc[slot_c] of the thread's
+// right-hand side (blockIdx.y).  A system whose stopping test fired at an EARLIER iteration (conv[rhs] in [0, iter)) is
+// frozen: the host runs one iteration ahead of the residuals it has read, and other systems of a batch may still iterate.
 template <typename R>
 __global__ void __launch_bounds__(128) cg_xp_kernel(int Ls, int TS, unsigned nvec_site, typename V5<R>::V* __restrict__ x,
                                                     typename V5<R>::V* __restrict__ p,
                                                     const typename V5<R>::V* __restrict__ r,
                                                     typename V5<R>::V* __restrict__ ap, const double* __restrict__ sc,
-                                                    int slot_c, int slot_d, int slot_cn, int init, R b5, R c5, R mf) {
+                                                    int slot_c, int slot_d, int slot_cn, int init, R b5, R c5, R mf,
+                                                    const int* __restrict__ conv, int iter) {
     using V = typename V5<R>::V;
     constexpr int K = V5<R>::K;
     const unsigned gid = blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= nvec_site) return;
+    const int rhs = blockIdx.y;
+    if (!init) {
+        const int cv = conv[rhs];
+        if (cv >= 0 && cv < iter) return;
+    }
     const unsigned per_tile = (unsigned)K * TS;
     const unsigned tile = gid / per_tile, j = gid - tile * per_tile;
     const int k = j / TS;
     const bool rev = (k >= K / 2);
-    const size_t base = (size_t)tile * Ls * per_tile + j;
+    const size_t base = ((size_t)tile * gridDim.y + rhs) * Ls * per_tile + j;
     R alpha = (R)0, beta = (R)0;
     if (!init) {
-        const double cc = sc[slot_c];
-        alpha = (R)(cc / sc[slot_d]);
-        beta = (R)(sc[slot_cn] / cc);
+        const double cc = sc[slot_c * MAXR + rhs];
+        alpha = (R)(cc / sc[slot_d * MAXR + rhs]);
+        beta = (R)(sc[slot_cn * MAXR + rhs] / cc);
     }
     const size_t olast = base + (size_t)(rev ? 0 : Ls - 1) * per_tile;
     V prev = r[olast];
@@ -230,35 +238,45 @@ __global__ void __launch_bounds__(128) cg_xp_kernel(int Ls, int TS, unsigned nve
 }
 
 dwf_status launch_cg_xp(dwf_ctx* c, void* x, void* p, const void* r, void* ap, int prec, int slot_c, int slot_d,
-                        int slot_cn, int init) {
+                        int slot_cn, int init, int iter) {
     const Geom& g = c->g;
     const int block = 128;
     if (prec == DWF_F64) {
         const unsigned nvec_site = (unsigned)g.Vh * 12;
-        cg_xp_kernel<double><<<(nvec_site + block - 1) / block, block, 0, c->stream>>>(
+        const dim3 grid((nvec_site + block - 1) / block, c->nrhs_cur);
+        cg_xp_kernel<double><<<grid, block, 0, c->stream>>>(
             g.Ls, g.TS, nvec_site, (double2*)x, (double2*)p, (const double2*)r, (double2*)ap, c->scalars, slot_c, slot_d,
-            slot_cn, init, c->b5, c->c5, c->mf);
+            slot_cn, init, c->b5, c->c5, c->mf, c->cg_conv, iter);
     } else {
         const unsigned nvec_site = (unsigned)g.Vh * 6;
-        cg_xp_kernel<float><<<(nvec_site + block - 1) / block, block, 0, c->stream>>>(
+        const dim3 grid((nvec_site + block - 1) / block, c->nrhs_cur);
+        cg_xp_kernel<float><<<grid, block, 0, c->stream>>>(
             g.Ls, g.TS, nvec_site, (float4*)x, (float4*)p, (const float4*)r, (float4*)ap, c->scalars, slot_c, slot_d,
-            slot_cn, init, (float)c->b5, (float)c->c5, (float)c->mf);
+            slot_cn, init, (float)c->b5, (float)c->c5, (float)c->mf, c->cg_conv, iter);
     }
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
     return DWF_OK;
 }
 
-// fixed-tree final reduction of the per-block partials into one device scalar
+// fixed-tree final reduction of the per-block partials into one device scalar per right-hand side (block = rhs):
+// partials[rhs * n + i] -> result[rhs].  With `target` set it is also the CG's stopping test (reading C8), kept on the
+// device: the first iteration at which |r|^2 <= target[rhs] is recorded in conv[rhs].
 __global__ void __launch_bounds__(1024) reduce_partials_kernel(const double* __restrict__ partials, int n,
-                                                               double* __restrict__ result) {
+                                                               double* __restrict__ result, const double* __restrict__ target,
+                                                               int* __restrict__ conv, int iter) {
+    const int rhs = blockIdx.x;
     double v = 0.0;
-    for (int i = threadIdx.x; i < n; i += 1024) v += partials[i];
+    for (int i = threadIdx.x; i < n; i += 1024) v += partials[(size_t)rhs * n + i];
     double tot = block_reduce_sum(v);
-    if (threadIdx.x == 0) *result = tot;
+    if (threadIdx.x == 0) {
+        result[rhs] = tot;
+        if (target != nullptr && conv[rhs] < 0 && tot <= target[rhs]) conv[rhs] = iter;
+    }
 }
 
 dwf_status ensure_partials(dwf_ctx* c, int n) {
+    n *= c->nrhs_cur;
     if (n <= c->npartials) return DWF_OK;
     if (c->partials) cudaFree(c->partials);
     c->partials = nullptr;
@@ -271,8 +289,10 @@ dwf_status ensure_partials(dwf_ctx* c, int n) {
     return DWF_OK;
 }
 
-dwf_status launch_reduce(dwf_ctx* c, int n, int slot) {
-    reduce_partials_kernel<<<1, 1024, 0, c->stream>>>(c->partials, n, c->scalars + slot);
+// n partials per right-hand side -> scalars[slot][rhs]; iter > 0: also the stopping test of CG iteration `iter`
+dwf_status launch_reduce(dwf_ctx* c, int n, int slot, int iter) {
+    reduce_partials_kernel<<<c->nrhs_cur, 1024, 0, c->stream>>>(c->partials, n, c->scalars + (size_t)slot * MAXR,
+                                                                iter > 0 ? c->cg_target : nullptr, c->cg_conv, iter);
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
     return DWF_OK;
@@ -287,13 +307,14 @@ static dwf_status launch_op5_t(dwf_ctx* c, void* out, const void* x, int op1, co
     const int Ls = g.Ls;
     const unsigned nvec_site = (unsigned)g.Vh * K;
     const int block = 128;
-    const int grid = (int)((nvec_site + block - 1) / block);
+    const int gridx = (int)((nvec_site + block - 1) / block);
+    const dim3 grid(gridx, c->nrhs_cur);
     const R* tabs = (sizeof(R) == 8) ? (const R*)c->dtab.d64 : (const R*)c->dtab.d32;
     const R* T1 = tabs + (size_t)op1 * 2 * Ls * Ls;
     const R* T2 = (mode == 2) ? tabs + (size_t)op2 * 2 * Ls * Ls : nullptr;
     double* partials = nullptr;
     if (norm_slot >= 0) {
-        dwf_status st = ensure_partials(c, grid);
+        dwf_status st = ensure_partials(c, gridx);
         if (st != DWF_OK) return st;
         partials = c->partials;
     }
@@ -314,7 +335,7 @@ static dwf_status launch_op5_t(dwf_ctx* c, void* out, const void* x, int op1, co
 #undef DWF_OP5_LAUNCH
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
-    if (norm_slot >= 0) return launch_reduce(c, grid, norm_slot);
+    if (norm_slot >= 0) return launch_reduce(c, gridx, norm_slot, 0);
     return DWF_OK;
 }
 
@@ -350,8 +371,8 @@ __global__ void __launch_bounds__(128) cg_r_kernel(int Ls, int TS, unsigned nvec
         const unsigned tile = gid / per_tile, j = gid - tile * per_tile;
         const int k = j / TS;
         const bool rev = (k < K / 2);          // daggered: P+ components walk s downwards
-        const size_t base = (size_t)tile * Ls * per_tile + j;
-        const R alpha = (R)(sc[slot_c] / sc[slot_d]);
+        const size_t base = ((size_t)tile * gridDim.y + blockIdx.y) * Ls * per_tile + j;     // blockIdx.y: right-hand side
+        const R alpha = (R)(sc[slot_c * MAXR + blockIdx.y] / sc[slot_d * MAXR + blockIdx.y]);
         const size_t olast = base + (size_t)(rev ? 0 : Ls - 1) * per_tile;
         V qprev = q[olast], dprev = d[olast];
         scalev(qprev, -mf);
@@ -374,17 +395,18 @@ __global__ void __launch_bounds__(128) cg_r_kernel(int Ls, int TS, unsigned nvec
         }
     }
     const double tot = block_reduce_sum(nrm);
-    if (threadIdx.x == 0) partials[blockIdx.x] = tot;
+    if (threadIdx.x == 0) partials[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = tot;
 }
 
 dwf_status launch_cg_r(dwf_ctx* c, void* r, const void* q, const void* d, double yscale, int prec, int slot_c, int slot_d,
-                       int norm_slot) {
+                       int norm_slot, int iter) {
     const Geom& g = c->g;
     const double bee = 1.0 + c->b5 * (4.0 - c->M5), cee = 1.0 - c->c5 * (4.0 - c->M5);
     const int block = 128;
     const unsigned nvec_site = (unsigned)g.Vh * (prec == DWF_F64 ? 12 : 6);
-    const int grid = (int)((nvec_site + block - 1) / block);
-    dwf_status st = ensure_partials(c, grid);
+    const int gridx = (int)((nvec_site + block - 1) / block);
+    const dim3 grid(gridx, c->nrhs_cur);
+    dwf_status st = ensure_partials(c, gridx);
     if (st != DWF_OK) return st;
     if (prec == DWF_F64)
         cg_r_kernel<double><<<grid, block, 0, c->stream>>>(g.Ls, g.TS, nvec_site, (double2*)r, (const double2*)q,
@@ -397,6 +419,6 @@ dwf_status launch_cg_r(dwf_ctx* c, void* r, const void* q, const void* d, double
                                                           (float)c->mf, c->partials);
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
-    return launch_reduce(c, grid, norm_slot);
+    return launch_reduce(c, gridx, norm_slot, iter);
 }
 }  // namespace dwf

@@ -226,7 +226,8 @@ __global__ void convert_kernel(Geom g, RD* __restrict__ dst, const RS* __restric
 }
 
 dwf_status launch_convert(dwf_ctx* c, void* dst, int dprec, const void* src, int sprec, size_t nhalf_fields) {
-    const Geom& g = c->g;
+    Geom g = c->g;
+    g.Ls *= c->nrhs_cur;       // batched field: one long fifth dimension (dwf_internal.h)
     const long long n = (long long)g.Vh * g.Ls * 6;
     const int block = 256;
     const int grid = (int)((n + block - 1) / block);
@@ -248,7 +249,8 @@ dwf_status launch_convert(dwf_ctx* c, void* dst, int dprec, const void* src, int
 }
 
 dwf_status launch_add_f32_to_f64(dwf_ctx* c, void* x64, const void* e32, size_t) {
-    const Geom& g = c->g;
+    Geom g = c->g;
+    g.Ls *= c->nrhs_cur;
     const long long n = (long long)g.Vh * g.Ls * 6;
     const int block = 256;
     const int grid = (int)((n + block - 1) / block);

@@ -18,6 +18,14 @@ namespace dwf {
 // Gauge, per OUTPUT parity: vec index = ((tile * 8 + leg) * KG + kg) * TS + lane, leg = 2*mu + dir,
 // dir 0: W = U_mu(x) (forward), dir 1: W = U_mu(x-mu)^dag (backward); 12 (rows 0,1) or 18 reals.
 // ---------------------------------------------------------------------------------------------
+// Batched ("multi right-hand side") fields: N systems that share one gauge field are stored as ONE
+// native field whose fifth dimension is N*Ls long, slice index rhs*Ls + s:
+//     vec index = (((tile * N + rhs) * Ls + s) * K + k) * TS + lane
+// The Dhop kernels do not look at s, so they run on such a field with Ls := N*Ls and load the links of a tile once for all
+// N*Ls slices; the column kernels and the Dhop epilogue take N and the physical Ls (the -mf walls sit at s = 0, Ls-1 of
+// every system).  Scalar slot `slot` of system `rhs` is scalars[slot * MAXR + rhs].
+constexpr int MAXR = 16;
+
 struct Geom {
     int L[4];    // lattice extents
     int T[4];    // tile extents
@@ -61,6 +69,7 @@ struct dwf_ctx {
     int dhop_grid = 0;     // CTAs of the persistent TMA kernel (0 = SMs x resident CTAs)
     int fuse = 1;          // Mpc / CG through the Dhop kernel's fused 5-D epilogues when the TMA kernel applies (0: separate op5 kernels)
     int dhop_dynamic = 1;  // TMA kernel tile scheduling: 1 global in-order queue (default), 0 static round-robin (always used by the fused launches, which reduce)
+    int dhop_l2hint = 0;   // TMA kernel L2 hints: bit 0 t-slab retention along the sweep, bit 1 links evict_first
     int dhop_skip = 0;     // debug only (traffic attribution): halo regions the TMA kernel does not load
     int dhop_order = 0;    // tile traversal of the TMA kernel: blob extents in tiles as digits (0 = default), dwf_dhop_tma.cu
     int dhop_order_axes = 0;   // blob path, fastest-first axis digits
@@ -74,6 +83,7 @@ struct dwf_ctx {
     double inner_tol = 1e-4;
     int max_restarts = 20;
     cudaStream_t stream = nullptr;
+    int device = 0;        // CUDA device the context was created on; every ABI call runs with it current (DeviceGuard)
     bool gauge_set = false;
     bool geom_frozen = false;
     // gauge copies [parity]
@@ -96,8 +106,19 @@ struct dwf_ctx {
     size_t ms_p_bytes = 0;
     double* partials = nullptr;  // per-block reduction partials
     int npartials = 0;
-    double* scalars = nullptr;   // device scalars
-    double* scalars_host = nullptr;  // pinned
+    double* scalars = nullptr;   // device scalars [NSLOTS][MAXR]
+    double* scalars_host = nullptr;  // pinned, same shape
+    // device-side stopping test of the CG (one entry per right-hand side): cg_target = tol^2 |b|^2, cg_conv = first
+    // iteration with |r|^2 <= target (-1: none yet).  The host runs one iteration ahead of what it has read back.
+    double* cg_target = nullptr;     // device [MAXR]
+    int* cg_conv = nullptr;          // device [MAXR]
+    double* cn_ring = nullptr;       // pinned [CG_RING][MAXR]: |r|^2 of the last iterations
+    cudaEvent_t cg_ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    // workspace of the batched (multi right-hand side) calls: NWS fields of mrhs_cap systems per precision
+    void* wsm64[10] = {};
+    void* wsm32[10] = {};
+    int mrhs_cap = 0;
+    int nrhs_cur = 1;      // right-hand sides of the call in progress (1 outside the *_mrhs entry points)
     void* stage_dev[2] = {nullptr, nullptr};  // staging for *_host calls
     size_t stage_bytes[2] = {0, 0};
     long long launches = 0;
@@ -116,14 +137,34 @@ namespace dwf {
 // geometry as seen by fields of one precision: fp64 fields of 4^4 tiles are stored in the XOR-rotated lane order that makes
 // the fp64 Dhop kernel's shared-memory accesses conflict-free; fp32 fields keep the plain order (its kernel has no
 // registers left for the extra face gathers that order needs).  dwf_convert and x64 += e32 permute the lanes.
-inline Geom geom_prec(const dwf_ctx* c, int prec) {
+inline Geom geom_prec(const dwf_ctx* c, int prec, int nrhs = 1) {
     Geom g = c->g;
     g.swz = (prec == DWF_F64) ? c->swz64 : 0;
+    g.Ls *= nrhs;          // batched field: the Dhop kernels see one long fifth dimension
     return g;
 }
 
 inline size_t half_vecs(const Geom& g, int prec) { return (size_t)g.Vh * g.Ls * (prec == DWF_F64 ? 12 : 6); }
 inline size_t half_bytes(const Geom& g, int prec) { return half_vecs(g, prec) * 16; }
+
+// cudaFuncSetAttribute(MaxDynamicSharedMemorySize) is per device: one bit per device ordinal and kernel instantiation
+inline bool attr_needed(unsigned long long& done_mask, int device) {
+    const unsigned long long bit = 1ull << (device & 63);
+    if (done_mask & bit) return false;
+    done_mask |= bit;
+    return true;
+}
+
+// makes the context's device current for the duration of an ABI call and restores the caller's device afterwards
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(const dwf_ctx* c) {
+        if (!c) return;
+        int cur = 0;
+        if (cudaGetDevice(&cur) == cudaSuccess && cur != c->device && cudaSetDevice(c->device) == cudaSuccess) prev = cur;
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 #define DWF_CUDA_CHECK(ctx, expr)                                                            \
     do {                                                                                     \
@@ -148,7 +189,7 @@ dwf_status launch_convert(dwf_ctx* c, void* dst, int dprec, const void* src, int
 // BLAS-1 on native half fields; scalar slots index c->scalars
 dwf_status launch_norm2(dwf_ctx* c, const void* v, int prec, size_t nreal, int slot);
 dwf_status launch_cg_update(dwf_ctx* c, void* x, void* r, const void* p, const void* z, int prec, size_t nreal,
-                            int slot_c, int slot_d, int slot_cn);            // x+=a p; r-=a z; cn=|r|^2, a=c/d
+                            int slot_c, int slot_d, int slot_cn, int iter);  // x+=a p; r-=a z; cn=|r|^2, a=c/d (iter: stopping test)
 dwf_status launch_xpay(dwf_ctx* c, void* p, const void* r, int prec, size_t nreal, int slot_cn, int slot_c);  // p=r+(cn/c)p
 dwf_status launch_axpy(dwf_ctx* c, void* y, const void* x, double a, int prec, size_t nreal);  // y += a x
 dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int prec, size_t nreal);  // out = a - b
@@ -159,7 +200,7 @@ dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t 
 dwf_status launch_lincomb3(dwf_ctx* c, void* out, const void* x, const void* y, const void* z, double a, double b, double cc,
                            int prec, size_t nreal);   // out = a x + b y + cc z
 dwf_status ensure_partials(dwf_ctx* c, int n);
-dwf_status launch_reduce(dwf_ctx* c, int n, int slot);
+dwf_status launch_reduce(dwf_ctx* c, int n, int slot, int iter = 0);   // iter > 0: also the CG stopping test of that iteration
 void build_tables(dwf_ctx* c);
 dwf_status pipe_tables_upload(dwf_ctx* c);
 void pipe_tables_free(dwf_ctx* c);
@@ -174,14 +215,16 @@ dwf_status launch_dhop_fused(dwf_ctx* c, void* out, const void* in, int out_pari
                              int norm_slot);
 // r -= (sc[slot_c]/sc[slot_d]) (Mee^dag q + yscale A^dag d); |r|^2 -> scalars[norm_slot]   (dwf_fived.cu)
 dwf_status launch_cg_r(dwf_ctx* c, void* r, const void* q, const void* d, double yscale, int prec, int slot_c, int slot_d,
-                       int norm_slot);
+                       int norm_slot, int iter);
 // x += a p (a = sc[slot_c]/sc[slot_d]); p = r + b p (b = sc[slot_cn]/sc[slot_c]); ap = A p.  init: p = r, ap = A p only.
+// iter: CG iteration this launch belongs to (systems that converged before it are left untouched)
 dwf_status launch_cg_xp(dwf_ctx* c, void* x, void* p, const void* r, void* ap, int prec, int slot_c, int slot_d,
-                        int slot_cn, int init);
+                        int slot_cn, int init, int iter);
 dwf_status dhop_time_begin(dwf_ctx* c);
 dwf_status dhop_time_end(dwf_ctx* c, double alg_bytes);
 dwf_status dhop_timing_flush(dwf_ctx* c);   // synchronises the stream, folds recorded event pairs into dhop_ms
 
 enum { SLOT_C = 0, SLOT_D, SLOT_CN, SLOT_B, SLOT_T0, SLOT_T1, NSLOTS = 16 };
+constexpr int CG_RING = 4;
 
 }  // namespace dwf
