@@ -496,9 +496,12 @@ dwf_status dwf_create(dwf_ctx** out, const int dims[4], int Ls, double M5, doubl
         dwf_destroy(c);
         return DWF_ENOMEM;
     }
-    cudaMemcpy(c->dtab.d64, h64.data(), nt * sizeof(double), cudaMemcpyHostToDevice);
-    cudaMemcpy(c->dtab.d32, h32.data(), nt * sizeof(float), cudaMemcpyHostToDevice);
-    if (cudaGetLastError() != cudaSuccess) { dwf_destroy(c); return DWF_ECUDA; }
+    if (cudaMemcpy(c->dtab.d64, h64.data(), nt * sizeof(double), cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(c->dtab.d32, h32.data(), nt * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError();
+        dwf_destroy(c);
+        return DWF_ECUDA;
+    }
     *out = c;
     return DWF_OK;
 }
@@ -570,7 +573,6 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
         if (c->gauge_set) DWF_TRY(tma_state_build(c));
     }
     else if (k == "dhop_skip") c->dhop_skip = (int)val;
-    else if (k == "dhop_l2hint") c->dhop_l2hint = (int)val;
     else if (k == "dhop_nst") { if (val != 2 && val != 3) return DWF_EINVAL; c->dhop_nst = (int)val; }
 #endif
     else if (k == "time_dhop") {       // (re)start per-launch event timing of the Dhop kernel

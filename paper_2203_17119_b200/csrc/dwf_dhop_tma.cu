@@ -223,20 +223,12 @@ std::vector<uint32_t> build_order(const Geom& g, int code, int axes_code) {
     for (int ib = 0; ib < nblobs; ++ib) {
         int bc[4];
         blob_coords(ib, bc);
-        // t-sweep direction of this blob (bits 30-31 of its entries: 1 = the next blob is the +t neighbour, 2 = the -t one, 0 = neither):
-        // tells the producer which t-slabs the NEXT round will read again (L2 retention hints)
-        uint32_t dirflag = 0;
-        if (B[3] == 1 && ib + 1 < nblobs) {
-            int nb[4];
-            blob_coords(ib + 1, nb);
-            if (nb[0] == bc[0] && nb[1] == bc[1] && nb[2] == bc[2]) dirflag = (nb[3] == bc[3] + 1) ? 1u : (nb[3] == bc[3] - 1 ? 2u : 0u);
-        }
         for (int t = 0; t < B[3]; ++t)
             for (int z = 0; z < B[2]; ++z)
                 for (int y = 0; y < B[1]; ++y)
                     for (int x = 0; x < B[0]; ++x) {
                         const int c[4] = {bc[0] * B[0] + x, bc[1] * B[1] + y, bc[2] * B[2] + z, bc[3] * B[3] + t};
-                        o.push_back((uint32_t)tile_index(g, c) | (dirflag << 30));
+                        o.push_back((uint32_t)tile_index(g, c));
                     }
     }
     return o;
@@ -300,29 +292,33 @@ dwf_status tma_state_build(dwf_ctx* c) {
         if (g.T[mu] != 4) return DWF_OK;
     if (!encode_fn()) return DWF_OK;
     TmaState* s = new TmaState();
-    c->tma = s;
-    cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, c->device);
-    // fp64 tables first (K = 12, XOR-rotated lane order), fp32 second (K = 6, plain order)
-    TmaTables t64 = build_tma_tables_swz(12), t32 = build_tma_tables_plain(6);
-    std::vector<uint16_t> off(t64.off);
-    off.insert(off.end(), t32.off.begin(), t32.off.end());
-    const std::vector<uint16_t>& gdst = t64.gdst;
-    std::vector<uint32_t> order = build_order(g, c->dhop_order, c->dhop_order_axes);
-    DWF_CUDA_CHECK(c, cudaMalloc(&s->off, off.size() * sizeof(uint16_t)));
-    DWF_CUDA_CHECK(c, cudaMalloc(&s->xsrc, t32.xsrc.size()));
-    DWF_CUDA_CHECK(c, cudaMalloc(&s->xdst, t32.xdst.size() * sizeof(uint16_t)));
-    DWF_CUDA_CHECK(c, cudaMalloc(&s->gsrc, t64.gsrc.size()));
-    DWF_CUDA_CHECK(c, cudaMalloc(&s->gdst, gdst.size() * sizeof(uint16_t)));
-    DWF_CUDA_CHECK(c, cudaMalloc(&s->order, order.size() * sizeof(uint32_t)));
-    DWF_CUDA_CHECK(c, cudaMemcpy(s->off, off.data(), off.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
-    DWF_CUDA_CHECK(c, cudaMemcpy(s->xsrc, t32.xsrc.data(), t32.xsrc.size(), cudaMemcpyHostToDevice));
-    DWF_CUDA_CHECK(c, cudaMemcpy(s->xdst, t32.xdst.data(), t32.xdst.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
-    DWF_CUDA_CHECK(c, cudaMemcpy(s->gsrc, t64.gsrc.data(), t64.gsrc.size(), cudaMemcpyHostToDevice));
-    DWF_CUDA_CHECK(c, cudaMemcpy(s->gdst, gdst.data(), gdst.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
-    DWF_CUDA_CHECK(c, cudaMemcpy(s->order, order.data(), order.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
-    DWF_CUDA_CHECK(c, cudaMalloc(&s->counters, 4 * sizeof(int)));
-    DWF_CUDA_CHECK(c, cudaMemset(s->counters, 0, 4 * sizeof(int)));
-    return DWF_OK;
+    c->tma = s;            // tma_state_free releases a half-built state; published for launches only on success (below)
+    dwf_status st = [&]() -> dwf_status {
+        cudaDeviceGetAttribute(&s->num_sms, cudaDevAttrMultiProcessorCount, c->device);
+        // fp64 tables first (K = 12, XOR-rotated lane order), fp32 second (K = 6, plain order)
+        TmaTables t64 = build_tma_tables_swz(12), t32 = build_tma_tables_plain(6);
+        std::vector<uint16_t> off(t64.off);
+        off.insert(off.end(), t32.off.begin(), t32.off.end());
+        const std::vector<uint16_t>& gdst = t64.gdst;
+        std::vector<uint32_t> order = build_order(g, c->dhop_order, c->dhop_order_axes);
+        DWF_CUDA_CHECK(c, cudaMalloc(&s->off, off.size() * sizeof(uint16_t)));
+        DWF_CUDA_CHECK(c, cudaMalloc(&s->xsrc, t32.xsrc.size()));
+        DWF_CUDA_CHECK(c, cudaMalloc(&s->xdst, t32.xdst.size() * sizeof(uint16_t)));
+        DWF_CUDA_CHECK(c, cudaMalloc(&s->gsrc, t64.gsrc.size()));
+        DWF_CUDA_CHECK(c, cudaMalloc(&s->gdst, gdst.size() * sizeof(uint16_t)));
+        DWF_CUDA_CHECK(c, cudaMalloc(&s->order, order.size() * sizeof(uint32_t)));
+        DWF_CUDA_CHECK(c, cudaMemcpy(s->off, off.data(), off.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        DWF_CUDA_CHECK(c, cudaMemcpy(s->xsrc, t32.xsrc.data(), t32.xsrc.size(), cudaMemcpyHostToDevice));
+        DWF_CUDA_CHECK(c, cudaMemcpy(s->xdst, t32.xdst.data(), t32.xdst.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        DWF_CUDA_CHECK(c, cudaMemcpy(s->gsrc, t64.gsrc.data(), t64.gsrc.size(), cudaMemcpyHostToDevice));
+        DWF_CUDA_CHECK(c, cudaMemcpy(s->gdst, gdst.data(), gdst.size() * sizeof(uint16_t), cudaMemcpyHostToDevice));
+        DWF_CUDA_CHECK(c, cudaMemcpy(s->order, order.data(), order.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+        DWF_CUDA_CHECK(c, cudaMalloc(&s->counters, 4 * sizeof(int)));
+        DWF_CUDA_CHECK(c, cudaMemset(s->counters, 0, 4 * sizeof(int)));
+        return DWF_OK;
+    }();
+    if (st != DWF_OK) tma_state_free(c);      // never leave half-built tables behind: later launches would dereference them
+    return st;
 }
 
 // three tensor maps over one native half field: [0] t-slabs (512-byte rows), [1] z faces (128-byte rows),
@@ -407,23 +403,6 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map
 __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, int c3, uint32_t bar) {
     asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4, %5}], [%6];"
                  ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void tma_load_3d_hint(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2, uint32_t bar, uint64_t pol) {
-    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1, {%2, %3, %4}], [%5], %6;"
-                 ::"r"(dst), "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(pol) : "memory");
-}
-__device__ __forceinline__ uint64_t policy_evict_last() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ uint64_t policy_evict_first() {
-    uint64_t p;
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
-    return p;
-}
-__device__ __forceinline__ void l2_prefetch_bulk_hint(const void* p, uint32_t bytes, uint64_t pol) {
-    asm volatile("cp.async.bulk.prefetch.L2.global.L2::cache_hint [%0], %1, %2;" ::"l"(p), "r"(bytes), "l"(pol) : "memory");
 }
 __device__ __forceinline__ void l2_prefetch(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void l2_prefetch_bulk(const void* p, uint32_t bytes) {
@@ -548,7 +527,6 @@ struct TmaArgs {
     const uint32_t* order;    // [ntiles]
     int* counters;            // [3] queue / done / round-arrival counters
     EpiArgs epi;
-    int l2hint;               // bit 0: t-slab retention hints along the sweep, bit 1: links prefetched evict_first
     int skip;                 // debug: bit r set = do not load halo region r (4..11); results are then wrong, traffic only
     int mode;                 // 0: static round-robin, 1: global in-order queue
     int dagger;
@@ -622,10 +600,8 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                 if (lane == 0) v = atomicAdd(a.counters, 1) + (int)gridDim.x;
                 it_next = __shfl_sync(0xffffffffu, v, 0);
             }
-            const uint32_t oent = a.order[it];
-            const int tile = (int)(oent & 0x3fffffffu);
-            const int tdir = (a.l2hint & 1) ? (int)(oent >> 30) : 0;      // 1: the next round reads the +t neighbours, 2: the -t ones
-            const int tile_next = (it_next < ntiles) ? (int)(a.order[it_next] & 0x3fffffffu) : -1;
+            const int tile = (int)a.order[it];
+            const int tile_next = (it_next < ntiles) ? (int)a.order[it_next] : -1;
             int tc[4];
             tile_coords(g, tile, tc);
             int nt[8];
@@ -650,31 +626,15 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                 if (lane == 0) {
                     // next tile's links -> L2, issued with this tile's last slice: the consumers want them NST slices
                     // later (issued a whole tile ahead they were evicted again before use and fetched twice)
-                    if (s == Ls - 1 && tile_next >= 0) {
-                        const V* wn = reinterpret_cast<const V*>(a.W) + (size_t)tile_next * 8 * KG * TSV;
-                        if (a.l2hint & 2) l2_prefetch_bulk_hint(wn, 8 * KG * TSV * 16, policy_evict_first());
-                        else l2_prefetch_bulk(wn, 8 * KG * TSV * 16);
-                    }
+                    if (s == Ls - 1 && tile_next >= 0)
+                        l2_prefetch_bulk(reinterpret_cast<const V*>(a.W) + (size_t)tile_next * 8 * KG * TSV, 8 * KG * TSV * 16);
                     const int nskip = __popc(SKIPM & (GATHER_Y ? 0x0f0 : 0x3f0));
                     mbar_arrive_expect_tx(full, (NTMA - nskip) * REGION_BYTES);
                     const int row_own = (tile * Ls + s) * K;
-                    if (tdir == 0) {
 #pragma unroll
-                        for (int tt = 0; tt < 4; ++tt) tma_load_3d(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full);
-                        if (!(SKIPM & 0x010)) tma_load_3d(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full);
-                        if (!(SKIPM & 0x020)) tma_load_3d(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full);
-                    } else {
-                        // the t sweep reads two slabs of this working set again one round later (the leading own slab as the
-                        // next tile's trailing face, the leading face as its own slab): keep those in L2, drop the trailing ones
-                        const uint64_t keep = policy_evict_last(), drop = policy_evict_first();
-                        const bool up = (tdir == 1);
-                        tma_load_3d_hint(base + 0 * REGION_BYTES, &map_slab, 0, 0, row_own, full, up ? drop : keep);
-                        tma_load_3d(base + 1 * REGION_BYTES, &map_slab, 0, 1, row_own, full);
-                        tma_load_3d(base + 2 * REGION_BYTES, &map_slab, 0, 2, row_own, full);
-                        tma_load_3d_hint(base + 3 * REGION_BYTES, &map_slab, 0, 3, row_own, full, up ? keep : drop);
-                        if (!(SKIPM & 0x010)) tma_load_3d_hint(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full, up ? keep : drop);
-                        if (!(SKIPM & 0x020)) tma_load_3d_hint(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full, up ? drop : keep);
-                    }
+                    for (int tt = 0; tt < 4; ++tt) tma_load_3d(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full);
+                    if (!(SKIPM & 0x010)) tma_load_3d(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full);
+                    if (!(SKIPM & 0x020)) tma_load_3d(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full);
                     if (!(SKIPM & 0x040)) tma_load_4d(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full);
                     if (!(SKIPM & 0x080)) tma_load_4d(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full);
                     if (!GATHER_Y) {
@@ -725,7 +685,7 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
     const R dsgn = a.dagger ? (R)-1 : (R)1;
     uint32_t n = 0, j = 0, nred = 0;
     double nrm = 0.0;
-    int tile = (int)(a.order[blockIdx.x] & 0x3fffffffu);
+    int tile = (int)a.order[blockIdx.x];
     while (tile >= 0) {
         int tile_next = -1;
         const int tct = tile / (g.NT[0] * g.NT[1] * g.NT[2]);
@@ -907,7 +867,6 @@ static dwf_status fill_args(dwf_ctx* c, TmaArgs& a, void* out, const void* in, i
 #ifdef DWF_PROBE
     a.skip = c->dhop_skip;
 #endif
-    a.l2hint = c->dhop_l2hint;
     a.dagger = dagger;
     a.epi.mode = EPI_NONE;
     return DWF_OK;

@@ -45,9 +45,50 @@ __global__ void gauge_prep_kernel(Geom g, const double* __restrict__ U, R* __res
     }
 }
 
+// max over all links of |row2 - conj(row0 x row1)|_inf: what 2-row compression (reading C10) would get wrong.
+// Non-negative doubles order like their bit patterns, so the maximum is an integer atomicMax.
+__global__ void su3_defect_kernel(const double* __restrict__ U, long long nlinks, unsigned long long* __restrict__ worst) {
+    double d = 0.0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < nlinks; i += (long long)gridDim.x * blockDim.x) {
+        const double* u = U + i * 18;
+        for (int cidx = 0; cidx < 3; ++cidx) {
+            const int a = (cidx + 1) % 3, b = (cidx + 2) % 3;
+            const double re = (u[2 * a] * u[6 + 2 * b] - u[2 * a + 1] * u[6 + 2 * b + 1]) - (u[2 * b] * u[6 + 2 * a] - u[2 * b + 1] * u[6 + 2 * a + 1]);
+            const double im = (u[2 * a] * u[6 + 2 * b + 1] + u[2 * a + 1] * u[6 + 2 * b]) - (u[2 * b] * u[6 + 2 * a + 1] + u[2 * b + 1] * u[6 + 2 * a]);
+            d = fmax(d, fmax(fabs(u[12 + 2 * cidx] - re), fabs(u[12 + 2 * cidx + 1] + im)));
+        }
+    }
+    if (!(d == d)) d = 1e300;      // NaN links
+    atomicMax(worst, (unsigned long long)__double_as_longlong(d));
+}
+
+// 2-row storage is exact only for SU(3) links: refuse anything else instead of silently computing another operator
+dwf_status check_su3(dwf_ctx* c, const double* Ucanon) {
+    unsigned long long* w = reinterpret_cast<unsigned long long*>(c->scalars + (size_t)SLOT_T1 * MAXR);
+    DWF_CUDA_CHECK(c, cudaMemsetAsync(w, 0, sizeof(*w), c->stream));
+    const long long nlinks = 2LL * c->g.Vh * 4;
+    su3_defect_kernel<<<148 * 4, 256, 0, c->stream>>>(Ucanon, nlinks, w);
+    c->launches++;
+    double d = 0.0;
+    DWF_CUDA_CHECK(c, cudaMemcpyAsync(&d, w, sizeof(d), cudaMemcpyDeviceToHost, c->stream));
+    DWF_CUDA_CHECK(c, cudaStreamSynchronize(c->stream));
+    if (d > 1e-10) {
+        char buf[200];
+        snprintf(buf, sizeof(buf), "set_gauge: links are not SU(3) (max |row2 - conj(row0 x row1)| = %.3e): 2-row compression "
+                                   "would change the operator; set option compress12 = 0", d);
+        c->err = buf;
+        return DWF_EINVAL;
+    }
+    return DWF_OK;
+}
+
 dwf_status launch_gauge_prep(dwf_ctx* c, const double* Ucanon) {
     const Geom& g = c->g;
     const int ng = c->compress12 ? 12 : 18;
+    if (c->compress12) {
+        dwf_status st = check_su3(c, Ucanon);
+        if (st != DWF_OK) return st;
+    }
     const int block = 128, grid = (g.Vh * 8 + block - 1) / block;
     const bool any_cut = c->cut[0] || c->cut[1] || c->cut[2] || c->cut[3];
     for (int set = 0; set < (any_cut && c->W64u[0] ? 2 : 1); ++set) {      // 0: with the Dirichlet cut, 1: without

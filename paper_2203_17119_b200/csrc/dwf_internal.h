@@ -68,8 +68,7 @@ struct dwf_ctx {
     int dhop_nst = 3;      // ring depth of the pipelined fp32 kernel
     int dhop_grid = 0;     // CTAs of the persistent TMA kernel (0 = SMs x resident CTAs)
     int fuse = 1;          // Mpc / CG through the Dhop kernel's fused 5-D epilogues when the TMA kernel applies (0: separate op5 kernels)
-    int dhop_dynamic = 1;  // TMA kernel tile scheduling: 1 global in-order queue (default), 0 static round-robin (always used by the fused launches, which reduce)
-    int dhop_l2hint = 0;   // TMA kernel L2 hints: bit 0 t-slab retention along the sweep, bit 1 links evict_first
+    int dhop_dynamic = 1;  // TMA kernel tile scheduling: 1 global in-order queue (default), 0 static round-robin (same results: every reduction is per tile)
     int dhop_skip = 0;     // debug only (traffic attribution): halo regions the TMA kernel does not load
     int dhop_order = 0;    // tile traversal of the TMA kernel: blob extents in tiles as digits (0 = default), dwf_dhop_tma.cu
     int dhop_order_axes = 0;   // blob path, fastest-first axis digits

@@ -80,8 +80,49 @@ def run(cfg, U, b_np, with_sweeps=True, max_iter=50000, extras=False):
             ms = _time(lambda: g.chebyshev(v, 0.0, 60.0, 16, prec, out=out), 3)
             rep[f"chebyshev16_{name}"] = {"ms": ms, "gflops": 16 * 2 * FLOP_MPC * n5h / ms / 1e6}
             del v, out
+    if extras:
+        rep["mrhs"] = mrhs_report(g, cfg, b)
     g.close()
     return rep
+
+
+def mrhs_report(g, cfg, b, counts=(1, 2, 4, 6), hbm_gbs=None):
+    """batched Dhop / Mpc^dag Mpc / CG against the number of right-hand sides.  Algorithmic bytes per
+    5-D site of the Dhop: 48 B + 8 g B / (nrhs Ls): the links are loaded once per tile for all nrhs * Ls slices."""
+    A = api
+    n5h = (cfg.V4 // 2) * cfg.Ls
+    rows = []
+    for n in counts:
+        try:
+            g.mrhs_reserve(n)
+        except api.DwfError as e:       # out of memory for this many systems
+            rows.append({"nrhs": n, "skipped": str(e)})
+            continue
+        row = {"nrhs": n}
+        for prec, name, B in ((A.F32, "f32", 4), (A.F64, "f64", 8)):
+            src = g.new_mrhs(n, prec).normal_()
+            dst = g.new_mrhs(n, prec)
+            ms = _time(lambda: g.dhop_mrhs(src, n, A.EVEN, False, prec, out=dst), 10)
+            by = n * n5h * 48 * B + (cfg.V4 // 2) * 8 * 12 * B
+            by_gauge = (cfg.V4 // 2) * 8 * 12 * B
+            ms2 = _time(lambda: g.mdagm_mrhs(src, n, prec, out=dst), 3)
+            row[name] = {"dhop_eo_ms": ms, "dhop_ms_per_rhs": ms / n, "dhop_gflops": FLOP_DHOP * n * n5h / ms / 1e6,
+                         "dhop_algorithmic_gbs": by / ms / 1e6, "gauge_share_of_bytes": by_gauge / by,
+                         "bytes_per_site": by / (n * n5h), "mdagm_ms": ms2, "mdagm_ms_per_rhs": ms2 / n,
+                         "mdagm_gflops": 2 * FLOP_MPC * n * n5h / ms2 / 1e6}
+            del src, dst
+        # n sources: the configured one and rescaled / operator-smoothed copies, so the systems differ
+        fields = [b] + [g.mdagm(b, A.F64) if j % 2 else b * (0.5 ** j) for j in range(1, n)]
+        bb = g.mrhs_gather(fields)
+        del fields
+        for mode, mname in ((A.CG_F64, "cg_f64"), (A.CG_MIXED, "cg_mixed")):
+            x, infos, st = g.cg_mrhs(bb, n, cfg.tol, 50000, mode)
+            row[mname] = {"status": int(st), "iters": [i["iters_total"] for i in infos], "seconds": infos[0]["seconds"],
+                          "seconds_per_rhs": infos[0]["seconds"] / n, "resid_true_max": max(i["resid_true"] for i in infos)}
+            del x
+        del bb
+        rows.append(row)
+    return rows
 
 
 def roofline_sweep(cfg, U, hbm_gbs):
