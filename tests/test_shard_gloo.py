@@ -24,7 +24,10 @@ def _free_port():
 
 
 def _worker(rank, world, port, out_dir):
-    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    # each rank's oracle gets its share of the cores (set before libgomp loads): two ranks with all cores each spin against
+    # one another and the test takes a minute instead of seconds
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world),
+                      OMP_NUM_THREADS=str(max(1, (os.cpu_count() or 2) // world)), OMP_WAIT_POLICY="passive")
     dist.init_process_group("gloo", rank=rank, world_size=world)
     try:
         from oracle.dwf_oracle import Oracle, solve_redblack
