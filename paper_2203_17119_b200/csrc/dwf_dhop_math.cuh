@@ -44,6 +44,19 @@ __device__ __forceinline__ void load_link(const typename VT<R>::V* __restrict__ 
     }
 }
 
+// row 2 of an SU(3) link from rows 0, 1 (reading C10): u[12..17] = conj(row0 x row1)
+template <typename R>
+__device__ __forceinline__ void third_row(R (&u)[18]) {
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const int a = (c + 1) % 3, b = (c + 2) % 3;
+        R ar = u[2 * a], ai = u[2 * a + 1], br = u[6 + 2 * b], bi = u[6 + 2 * b + 1];
+        R cr = u[2 * b], ci = u[2 * b + 1], dr = u[6 + 2 * a], di = u[6 + 2 * a + 1];
+        u[12 + 2 * c] = (ar * br - ai * bi) - (cr * dr - ci * di);
+        u[12 + 2 * c + 1] = -((ar * bi + ai * br) - (cr * di + ci * dr));
+    }
+}
+
 // ---- spin projection: h = upper two rows of (1 + SG*gamma_MU) psi ------------------------------
 // psi[(sp*3+c)*2+ri]; h[(hs*3+c)*2+ri]
 template <typename R, int MU, int SG>

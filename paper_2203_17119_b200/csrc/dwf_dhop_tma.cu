@@ -424,6 +424,17 @@ __device__ __forceinline__ double2 lds_v(const double2*, uint32_t a) {
 __device__ __forceinline__ void stcs_v(float4* p, const float4& v) { __stcs(p, v); }
 __device__ __forceinline__ void stcs_v(double2* p, const double2& v) { __stcs(p, v); }
 
+// global loads the compiler may not sink below the slice's shared-memory loads (both are volatile asm, kept in order)
+__device__ __forceinline__ float4 ldg_early(const float4* p) {
+    float4 v;
+    asm volatile("ld.global.nc.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ double2 ldg_early(const double2* p) {
+    double2 v;
+    asm volatile("ld.global.nc.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
+    return v;
+}
 __device__ __forceinline__ void pin_reg(float& v) { asm volatile("" : "+f"(v)); }
 __device__ __forceinline__ void pin_reg(double& v) { asm volatile("" : "+d"(v)); }
 __device__ __forceinline__ float shfl16(float v) { return __shfl_xor_sync(0xffffffffu, v, 16); }
@@ -553,7 +564,7 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
 
     extern __shared__ __align__(1024) unsigned char smem_raw[];
     __shared__ __align__(8) unsigned long long bars[2 * NST];   // full[NST], empty[NST]
-    __shared__ double wsum[2][4 * TPS];   // per-tile |.|^2 partials of the consumer warps (fused epilogue), double-buffered
+    __shared__ double wsum[4 * TPS];      // per-(system, tile) |.|^2 partials of the consumer warps (fused epilogue)
     __shared__ int next_of[4];     // slot j & 3, written before slice 0 of this CTA's j-th tile: the tile it takes after it (-1: none)
 
     const Geom& g = a.g;
@@ -685,15 +696,20 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
     }
     const int tt = site >> 5;
     const R dsgn = a.dagger ? (R)-1 : (R)1;
-    uint32_t n = 0, j = 0, nred = 0;
+    uint32_t n = 0, j = 0;
     double nrm = 0.0;
     int tile = (int)a.order[blockIdx.x];
     while (tile >= 0) {
         int tile_next = -1;
         const int tct = tile / (g.NT[0] * g.NT[1] * g.NT[2]);
         const int tglob = tct * 4 + tt;
-        // ---- links to registers (once per tile): rows 0,1 (+ row 2 rebuilt), antiperiodic sign folded in
+        // ---- links to registers (once per tile): rows 0,1 (+ row 2 rebuilt), antiperiodic sign folded in.
+        // REMAT (fp64 kernel with the fused epilogue): only rows 0, 1 stay in registers and row 2 is rebuilt in every slice
+        // (+18 % FP64 instructions) -- the 48 registers this frees hold the epilogue's 12 global loads, issued at the top of
+        // the slice instead of at its end where nothing hid their latency (long-scoreboard stalls 3.2 per issue before)
+        constexpr bool REMAT = (EPI != 0) && (sizeof(R) == 8) && (NG == 12);
         R u[LPT][18];
+        R tsgn = (R)1;                  // REMAT: antiperiodic sign of this lane's t leg, applied to the rebuilt row
         {
             const V* __restrict__ Wt = reinterpret_cast<const V*>(a.W) + (size_t)tile * 8 * KG * TSV + site;
 #pragma unroll
@@ -707,12 +723,14 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                     if (flip) {
 #pragma unroll
                         for (int i = 0; i < 18; ++i) u[j][i] = -u[j][i];
+                        tsgn = (R)-1;
                     }
                 }
-                // fp32: the rebuilt third row stays in registers for the whole tile: without this the compiler, short of
-                // registers, recomputes it from rows 0, 1 in every slice (+19 % FP instructions in the s loop: 1032 -> 870;
-                // the fp64 loop has no such recomputation)
-                if (NG == 12 && sizeof(R) == 4) {
+                // fp32, plain kernel: the rebuilt third row stays in registers for the whole tile: without this the compiler,
+                // short of registers, recomputes it from rows 0, 1 in every slice (+19 % FP instructions in the s loop:
+                // 1032 -> 870; the fp64 loop has no such recomputation).  Not in the fused kernel: there the registers the
+                // recomputation frees let the epilogue's global loads issue early (414 us vs 529 us with the rows pinned).
+                if (NG == 12 && sizeof(R) == 4 && EPI == 0) {
 #pragma unroll
                     for (int i = 12; i < 18; ++i) pin_reg(u[j][i]);
                 }
@@ -720,8 +738,8 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
         }
         V* __restrict__ outp = reinterpret_cast<V*>(a.out) + (size_t)tile * Ls * K * TSV + site;
         const V* __restrict__ xin_t = reinterpret_cast<const V*>(a.epi.xin) + (size_t)tile * Ls * K * TSV + site;
-        // fused epilogue on a batched field: sl = slice within its system (0 .. Ls0-1), rb = first slice of that system
-        int sl = 0, rb = 0;
+        // fused epilogue on a batched field: sl = slice within its system (0 .. Ls0-1); s - sl = first slice of that system
+        int sl = 0;
         for (int s = 0; s < Ls; ++s, ++n) {
             const uint32_t st = n % NST, ph = (n / NST) & 1;
             const uint32_t base = stage0 + st * STAGE_BYTES;
@@ -738,9 +756,21 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
 #pragma unroll
                     for (int k = 0; k < 6; ++k) {
                         l2_prefetch(xk + (size_t)s * (K * TSV) + k * TSV);
-                        l2_prefetch(xk + (size_t)(rb + a.epi.Ls0 - 1) * (K * TSV) + k * TSV);
+                        l2_prefetch(xk + (size_t)(s + a.epi.Ls0 - 1) * (K * TSV) + k * TSV);
                     }
                 }
+            }
+            // REMAT: this lane's epilogue operands (its chirality half of xin_s and of xin_{s-1} / xin_{s+1}) -> registers,
+            // requested here; ptxas places the loads as early as its register budget allows (in the exchange phase, well
+            // before their use; loading them one whole slice ahead spilled and was slower: 988 us vs 920 us)
+            V xcv[K / 2], xnv[K / 2];
+            if (REMAT && EPI != 0) {
+                const int Ls0e = a.epi.Ls0;
+                const V* xs_e = xin_t + (size_t)s * (K * TSV) + (sub ? K / 2 : 0) * TSV;
+                const int sn = sub ? ((sl + 1 < Ls0e) ? s + 1 : s + 1 - Ls0e) : ((sl > 0) ? s - 1 : s + Ls0e - 1);
+                const V* xn_e = xin_t + (size_t)sn * (K * TSV) + (sub ? K / 2 : 0) * TSV;
+#pragma unroll
+                for (int k = 0; k < K / 2; ++k) { xcv[k] = ldg_early(xs_e + k * TSV); xnv[k] = ldg_early(xn_e + k * TSV); }
             }
             R acc[24];
 #pragma unroll
@@ -752,6 +782,14 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                 const uint32_t p = base + myoff[j];
 #pragma unroll
                 for (int k = 0; k < K; ++k) unpackv(lds_v((const V*)nullptr, p + k * 512), psi + k * VW);
+                if (REMAT) {
+                    pin_reg(u[j][0]);                  // opaque: keeps the rebuild inside the slice loop
+                    third_row<R>(u[j]);
+                    if (mu == 3) {
+#pragma unroll
+                        for (int i = 12; i < 18; ++i) u[j][i] *= tsgn;
+                    }
+                }
                 if (j == 0) { proj_s<R, 0>(psi, sg, h); su3_mul<R>(u[j], h, gg); recon_s<R, 0, true>(gg, sg, acc); }
                 else if (mu == 0) { proj_s<R, 0>(psi, sg, h); su3_mul<R>(u[j], h, gg); recon_s<R, 0, false>(gg, sg, acc); }
                 else if (mu == 1) { proj_s<R, 1>(psi, sg, h); su3_mul<R>(u[j], h, gg); recon_s<R, 1, false>(gg, sg, acc); }
@@ -767,8 +805,8 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
             const R e_wm = (R)((sl > 0) ? a.epi.mcee : -a.epi.mf * a.epi.mcee);            // P+ : xin_{s-1}
             const R e_wp = (R)((sl + 1 < Ls0) ? a.epi.mcee : -a.epi.mf * a.epi.mcee);      // P- : xin_{s+1}
             const V* xs = xin_t + (size_t)s * (K * TSV);
-            const V* xm = xin_t + (size_t)((sl > 0) ? s - 1 : rb + Ls0 - 1) * (K * TSV);
-            const V* xp = xin_t + (size_t)((sl + 1 < Ls0) ? s + 1 : rb) * (K * TSV);
+            const V* xm = xin_t + (size_t)((sl > 0) ? s - 1 : s + Ls0 - 1) * (K * TSV);
+            const V* xp = xin_t + (size_t)((sl + 1 < Ls0) ? s + 1 : s + 1 - Ls0) * (K * TSV);
             if (TPS == 1) {
                 if constexpr (EPI != 0) {
 #pragma unroll
@@ -800,7 +838,9 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                     const R w = sub ? e_wp : e_wm;
 #pragma unroll
                     for (int k = 0; k < K / 2; ++k) {
-                        const V ov = vfma(e_scale, packv(mine + k * VW), vfma(w, ldg_v(xn_p + k * TSV), vmul(e_bee, ldg_v(xc_p + k * TSV))));
+                        const V xnk = REMAT ? xnv[k] : ldg_v(xn_p + k * TSV);
+                        const V xck = REMAT ? xcv[k] : ldg_v(xc_p + k * TSV);
+                        const V ov = vfma(e_scale, packv(mine + k * VW), vfma(w, xnk, vmul(e_bee, xck)));
                         nrm += vnorm2(ov);
                         stcs_v(o2 + k * TSV, ov);
                     }
@@ -816,19 +856,18 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                     if (a.epi.partials != nullptr) {
 #pragma unroll
                         for (int o2 = 16; o2 > 0; o2 >>= 1) nrm += __shfl_xor_sync(0xffffffffu, nrm, o2);
-                        if (lane == 0) wsum[nred & 1][cw] = nrm;
+                        if (lane == 0) wsum[cw] = nrm;
                         asm volatile("bar.sync 1, %0;" ::"n"(128 * TPS) : "memory");
                         if (ctid == 0) {
                             double t = 0.0;
 #pragma unroll
-                            for (int i = 0; i < NCW; ++i) t += wsum[nred & 1][i];
-                            a.epi.partials[(size_t)(rb / Ls0) * ntiles + tile] = t;
+                            for (int i = 0; i < NCW; ++i) t += wsum[i];
+                            a.epi.partials[(size_t)(s / Ls0) * ntiles + tile] = t;
                         }
+                        asm volatile("bar.sync 1, %0;" ::"n"(128 * TPS) : "memory");      // wsum is free again
                         nrm = 0.0;
-                        ++nred;
                     }
                     sl = 0;
-                    rb = s + 1;
                 }
             }
         }
