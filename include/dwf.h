@@ -140,7 +140,7 @@ dwf_status dwf_cg(dwf_ctx* ctx, void* x_dev, const void* b_dev, double tol, int 
  * site: 48 B + 8 g B / (N Ls), g = 12 or 18 reals, B = 4 or 8), and every other kernel of Mpc / CG runs once for the whole
  * batch.  dwf_cg_mrhs runs N independent CGs (readings C8 / C9 per system: own alpha, beta, stopping test, restarts) that
  * share the launches; a system that has converged is frozen while the others go on.  info: array of nrhs entries.
- * dwf_mrhs_reserve allocates the batched solver workspace (10 batched half fields per precision) ahead of time; otherwise
+ * dwf_mrhs_reserve allocates the batched solver workspace (8 batched half fields per precision) ahead of time; otherwise
  * the first batched Mpc / CG call with a larger nrhs does.  Status codes as the single-system calls (dwf_cg_mrhs:
  * DWF_ENOTCONV if any system has not converged at max_iter iterations).  out_parity: DWF_EVEN or DWF_ODD. */
 dwf_status dwf_mrhs_reserve(dwf_ctx* ctx, int nrhs);

@@ -33,8 +33,10 @@ dwf_status ws_alloc_all(dwf_ctx* c) {
     return DWF_OK;
 }
 
+const int NWSM = 8;       // the batched Mpc / CG paths use workspace fields 0..7 only (8, 9 belong to dwf_solve)
+
 void wsm_free(dwf_ctx* c) {
-    for (int i = 0; i < NWS; ++i) {
+    for (int i = 0; i < NWSM; ++i) {
         if (c->wsm64[i]) cudaFree(c->wsm64[i]);
         if (c->wsm32[i]) cudaFree(c->wsm32[i]);
         c->wsm64[i] = c->wsm32[i] = nullptr;
@@ -47,7 +49,7 @@ dwf_status wsm_reserve(dwf_ctx* c, int nrhs) {
     wsm_free(c);
     for (int prec = 0; prec < 2; ++prec) {
         void** arr = (prec == DWF_F64) ? c->wsm64 : c->wsm32;
-        for (int i = 0; i < NWS; ++i)
+        for (int i = 0; i < NWSM; ++i)
             if (cudaMalloc(&arr[i], half_bytes(c->g, prec) * nrhs) != cudaSuccess) {
                 cudaGetLastError();
                 wsm_free(c);

@@ -210,3 +210,28 @@ def test_c5_cg_first_iterations_and_mixed_solution(c5):
     true_res = np.sqrt(orc.norm2(odd - orc.mdagm(xs)) / orc.norm2(odd))
     assert true_res <= cfg.tol * (1 + 1e-6)
     assert abs(true_res - info["resid_true"]) <= 1e-6 * true_res + 1e-16
+
+
+def test_c4_batched_operators_and_cg_equal_the_single_system_path(c4):
+    """NEXT-3 at full size, in the launch configuration run_config --extras times: a batch of 3 systems through
+    dwf_dhop_mrhs / dwf_mdagm_mrhs equals the single-system kernels bit for bit (system 0 is the source the whole-field
+    oracle comparisons above use), and three CG iterations of the batch reproduce the single-system residuals exactly."""
+    import torch
+    A, g, odd = c4["api"], c4["g"], c4["odd"]
+    n = 3
+    nat = [g.pack(odd, A.F64, A.ODD)]
+    nat.append(nat[0] * 0.25)
+    nat.append(g.mdagm(nat[0], A.F64))
+    bb = g.mrhs_gather(nat)
+    for j, o in enumerate(g.mrhs_scatter(g.dhop_mrhs(bb, n, A.EVEN, False, A.F64), n)):
+        assert torch.equal(o, g.dhop(nat[j], A.EVEN, False, A.F64)), j
+    for j, o in enumerate(g.mrhs_scatter(g.mdagm_mrhs(bb, n, A.F64), n)):
+        assert torch.equal(o, g.mdagm(nat[j], A.F64)), j
+    bb32 = g.mrhs_gather([g.convert(v, A.F64, A.F32, A.ODD) for v in nat], A.F32)
+    for j, o in enumerate(g.mrhs_scatter(g.mdagm_mrhs(bb32, n, A.F32), n, A.F32)):
+        assert torch.equal(o, g.mdagm(g.convert(nat[j], A.F64, A.F32, A.ODD), A.F32)), j
+    x, infos, st = g.cg_mrhs(bb, n, 1e-30, 3)
+    assert st == A.ENOTCONV
+    for j, xs in enumerate(g.mrhs_scatter(x, n)):
+        x1, i1, _ = g.cg(nat[j], 1e-30, 3, A.CG_F64)
+        assert torch.equal(xs, x1) and infos[j]["resid_iter"] == i1["resid_iter"] and infos[j]["resid_true"] == i1["resid_true"]
