@@ -15,6 +15,10 @@
  *   coefficient tables and its solver workspace.  All work is enqueued on the context's CUDA
  *   stream (dwf_set_stream); only dwf_cg / dwf_solve / dwf_norm2 / *_host calls synchronise
  *   that stream, because they return scalars or host data.
+ *   A context is single-threaded and single-stream: its calls must not run concurrently with one another (the persistent
+ *   Dhop kernels share a tile-queue counter per context, the solver workspace is shared), and after dwf_set_stream the
+ *   caller orders the old stream's work before the new one's.  A context belongs to the CUDA device that was current at
+ *   dwf_create; every call makes that device current for its duration and restores the caller's afterwards.
  *   Every function returns a dwf_status; nothing throws or aborts across this boundary.
  *   dwf_last_error(ctx) gives a human-readable message for the last failure on ctx.
  *
