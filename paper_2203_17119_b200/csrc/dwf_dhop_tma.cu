@@ -22,6 +22,10 @@
 // on one, backward legs on the other), partial sums exchanged by warp shuffles, 1 CTA/SM; its fields use the
 // XOR-rotated lane order of dwf_layout.cuh and conflict-free face slots (build_tma_tables_swz).
 // EPI = 1 adds the last step of Mpc as an epilogue: out_s = Mee xin_s + scale (Dhop in)_s and its |.|^2.
+// Register budget (232 per consumer thread) decides the rest: the fp32 plain kernel pins the rebuilt third link rows so that
+// the compiler does not recompute them in every slice; the fp64 kernel with the epilogue does the opposite on purpose (rows
+// 0, 1 resident, row 2 rebuilt per slice) to have registers for its epilogue loads.  Batched fields (N systems, fifth
+// dimension N * Ls, dwf_internal.h) run through the same kernels with g.Ls = N * Ls; only the epilogue knows the physical Ls.
 #include <cuda.h>
 
 #include <algorithm>
