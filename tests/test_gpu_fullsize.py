@@ -235,3 +235,36 @@ def test_c4_batched_operators_and_cg_equal_the_single_system_path(c4):
     for j, xs in enumerate(g.mrhs_scatter(x, n)):
         x1, i1, _ = g.cg(nat[j], 1e-30, 3, A.CG_F64)
         assert torch.equal(xs, x1) and infos[j]["resid_iter"] == i1["resid_iter"] and infos[j]["resid_true"] == i1["resid_true"]
+
+
+def test_c4_mdagm_fp32_full_field(c4):
+    """The fp32 Schur operator at full size (the inner operator of the mixed-precision CG, reading C9) against the fp64
+    oracle on the fp32-rounded links and source: 1e-5 relative L2 per Dhop (north_star), 2x for Mpc^dag Mpc, and an
+    elementwise bar beside it."""
+    from oracle.dwf_oracle import Oracle
+    A, g, cfg, odd = c4["api"], c4["g"], c4["cfg"], c4["odd"]
+    U32 = c4["U"].astype(np.complex64).astype(np.complex128)
+    orc32 = Oracle(cfg.dims, cfg.Ls, cfg.M5, cfg.mf, cfg.b5, cfg.c5, antiperiodic_t=cfg.antiperiodic_t, cut=cfg.cut).set_gauge(U32)
+    src = odd.astype(np.complex64).astype(np.complex128)
+    got, want = g.unpack(g.mdagm(g.pack(src, A.F32, A.ODD), A.F32), A.F32, A.ODD), orc32.mdagm(src)
+    assert rel(got, want) < 2e-5 and relmax(got, want) < 4 * MAXTOL["f32"]
+
+
+def test_c5_adjoint_and_positivity_identities_on_the_gpu(c5):
+    """Properties that hold at any size (no oracle needed), at c5 in both precisions: <u, Mpc v> = <Mpc^dag u, v> (the dagger
+    kernels are the adjoints of the plain ones, reading C4'), and <v, Mpc^dag Mpc v> = |Mpc v|^2 > 0."""
+    import torch
+    A, g = c5["api"], c5["g"]
+    for P, tol in ((A.F64, 1e-12), (A.F32, 2e-5)):
+        u = g.new_native(P, A.ODD).normal_()
+        v = g.new_native(P, A.ODD).normal_()
+        dot = lambda a, b: complex(torch.dot(a.double(), b.double()).item())       # real dot of the re/im interleaved fields
+        # native fields are real arrays of (re, im) pairs in the same order for u and v: Re<u, w> = sum of products
+        mv, mdu = g.mpc(v, False, P), g.mpc(u, True, P)
+        lhs, rhs = dot(u, mv).real, dot(mdu, v).real
+        scale = float(torch.linalg.norm(u.double()) * torch.linalg.norm(mv.double()))
+        assert abs(lhs - rhs) <= tol * scale * 10, (P, lhs, rhs)
+        av = g.mdagm(v, P)
+        q = dot(v, av).real
+        n2 = g.norm2(mv, P, A.ODD)
+        assert q > 0 and abs(q - n2) <= tol * n2 * 10, (P, q, n2)
