@@ -527,6 +527,7 @@ dwf_status dwf_destroy(dwf_ctx* c) {
     pipe_tables_free(c);
     tma_state_free(c);
     if (c->ms_p) cudaFree(c->ms_p);
+    if (c->ms_state) cudaFree(c->ms_state);
     if (c->partials) cudaFree(c->partials);
     if (c->scalars) cudaFree(c->scalars);
     if (c->scalars_host) cudaFreeHost(c->scalars_host);
@@ -891,39 +892,51 @@ dwf_status dwf_multishift_cg(dwf_ctx* c, void* xv, const void* b, const double* 
     }
     DWF_CUDA_CHECK(c, cudaMemcpyAsync(r, b, hb, cudaMemcpyDeviceToDevice, c->stream));
     for (int i = 0; i < nshift; ++i) DWF_CUDA_CHECK(c, cudaMemcpyAsync(p + i * hb, b, hb, cudaMemcpyDeviceToDevice, c->stream));
+    // The scalar recurrences (alpha, beta, zeta_i and the update coefficients) live on the device (MsState); the stopping
+    // test is the CG's (cg_conv[0]) and the host runs one iteration ahead of the residual it has read, exactly as in
+    // cg_iterate: no stream synchronisation inside the loop.
     const double s0 = shifts[0], target = tol * tol * bn2;
-    double zeta[16], zeta_old[16], znew[16], ax[16], zr[16], bp[16];
-    for (int i = 0; i < nshift; ++i) zeta[i] = zeta_old[i] = 1.0;
-    double alpha_old = 1.0, beta_old = 0.0, cc = bn2, p0n2 = bn2;
-    int iters = 0;
-    while (cc > target && iters < max_iter) {
+    {
+        MsState h;
+        memset(&h, 0, sizeof(h));
+        h.n = nshift; h.s0 = s0; h.cc = bn2; h.p0n2 = bn2; h.alpha_old = 1.0; h.beta_old = 0.0;
+        for (int i = 0; i < nshift; ++i) { h.delta[i] = shifts[i] - s0; h.zeta[i] = h.zeta_old[i] = 1.0; }
+        if (!c->ms_state && cudaMalloc(&c->ms_state, sizeof(MsState)) != cudaSuccess) { cudaGetLastError(); c->err = "cudaMalloc(multishift state) failed"; return DWF_ENOMEM; }
+        DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->ms_state, &h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
+        CgRun run;
+        run.n = 1; run.target[0] = target; run.c[0] = bn2;
+        DWF_TRY(cg_upload_state(c, run, SLOT_C));          // cg_target[0], cg_conv[0] = -1 (synchronises: h may go out of scope)
+    }
+    double cc = bn2;
+    int iters = 0, k = 0, decided = 0;
+    bool done = (cc <= target);
+    auto decide = [&](int it, dwf_status* st) -> bool {
+        *st = DWF_OK;
+        if (cudaEventSynchronize(c->cg_ev[it % CG_RING]) != cudaSuccess) { c->err = "cudaEventSynchronize failed"; *st = DWF_ECUDA; return true; }
+        const double cn = c->cn_ring[(size_t)(it % CG_RING) * MAXR];
+        if (!(cn == cn)) { c->err = "multishift_cg: NaN residual"; *st = DWF_ECUDA; return true; }
+        cc = cn;
+        iters = it;
+        decided = it;
+        return cn <= target;
+    };
+    dwf_status lst = DWF_OK;
+    while (!done && k < max_iter) {
+        ++k;
         // q = Mpc p_0 (|q|^2 -> SLOT_D), z = Mpc^dag q;  d = <p_0, (A + s0) p_0> = |q|^2 + s0 |p_0|^2
         DWF_TRY(mpc_apply(c, q, p, 0, P, SLOT_D));
         DWF_TRY(mpc_apply(c, z, q, 1, P, -1));
-        double qn2;
-        DWF_TRY(read_slot(c, SLOT_D, &qn2));
-        const double d = qn2 + s0 * p0n2;
-        const double alpha = cc / d;
-        for (int i = 0; i < nshift; ++i) {
-            const double dl = shifts[i] - s0;
-            znew[i] = zeta[i] * zeta_old[i] * alpha_old /
-                      (alpha * beta_old * (zeta_old[i] - zeta[i]) + zeta_old[i] * alpha_old * (1.0 + dl * alpha));
-            ax[i] = alpha * znew[i] / zeta[i];
-        }
-        DWF_TRY(launch_ms_r(c, r, z, p, alpha, alpha * s0, n, SLOT_CN));        // r -= alpha (z + s0 p_0), |r|^2
-        double cn;
-        DWF_TRY(read_slot(c, SLOT_CN, &cn));
-        if (!(cn == cn)) { c->err = "multishift_cg: NaN residual"; return DWF_ECUDA; }
-        const double beta = cn / cc;
-        for (int i = 0; i < nshift; ++i) {
-            zr[i] = znew[i];
-            bp[i] = beta * (znew[i] / zeta[i]) * (znew[i] / zeta[i]);
-        }
-        DWF_TRY(launch_ms_update(c, x, p, r, n, nshift, ax, zr, bp, SLOT_T1));   // x_i += .. p_i ; p_i = .. ; |p_0|^2
-        DWF_TRY(read_slot(c, SLOT_T1, &p0n2));
-        for (int i = 0; i < nshift; ++i) { zeta_old[i] = zeta[i]; zeta[i] = znew[i]; }
-        alpha_old = alpha; beta_old = beta; cc = cn;
-        ++iters;
+        DWF_TRY(launch_ms_r(c, r, z, p, n, SLOT_D, SLOT_CN, k));               // alpha, zeta'; r -= alpha (z + s0 p_0); |r|^2, test
+        DWF_CUDA_CHECK(c, cudaMemcpyAsync(c->cn_ring + (size_t)(k % CG_RING) * MAXR, c->scalars + (size_t)SLOT_CN * MAXR, sizeof(double),
+                                          cudaMemcpyDeviceToHost, c->stream));
+        DWF_CUDA_CHECK(c, cudaEventRecord(c->cg_ev[k % CG_RING], c->stream));
+        DWF_TRY(launch_ms_update(c, x, p, r, n, SLOT_CN, SLOT_T1, k));         // beta; x_i += .. p_i ; p_i = .. ; |p_0|^2
+        if (k >= 2 && decide(k - 1, &lst)) { done = true; break; }
+    }
+    if (lst != DWF_OK) return lst;
+    while (!done && decided < k) {
+        done = decide(decided + 1, &lst);
+        if (lst != DWF_OK) return lst;
     }
     info->iters_total = iters;
     info->resid_iter = std::sqrt(cc / bn2);

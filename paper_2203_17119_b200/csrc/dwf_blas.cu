@@ -108,12 +108,49 @@ __global__ void __launch_bounds__(256) sub_kernel(typename VB<R>::V* __restrict_
         out[i] = axpyv((R)-1, b[i], a[i]);
 }
 
-// ---- multishift CG (dwf_multishift_cg): the residual step of the base system and one pass over all shifted systems
-// r -= a z + as0 p0 ; |r|^2
+// ---- multishift CG (dwf_multishift_cg): the scalar recurrences live on the device (MsState, one per context), so that the
+// loop needs no host round trip: two one-thread kernels form alpha / zeta / the update coefficients from the reduction
+// slots, the vector kernels read them from MsState.  The stopping test is the CG's (cg_conv[0], cg_target[0]).
+// before the residual step: d = |q|^2 + s0 |p_0|^2, alpha = c / d, zeta_i', ax_i = alpha zeta_i' / zeta_i
+__global__ void ms_alpha_kernel(MsState* __restrict__ st, const double* __restrict__ sc, int slot_d) {
+    if (threadIdx.x != 0) return;
+    const double d = sc[slot_d * MAXR] + st->s0 * st->p0n2;
+    const double alpha = st->cc / d;
+    st->alpha = alpha;
+    for (int i = 0; i < st->n; ++i) {
+        const double z = st->zeta[i], zo = st->zeta_old[i];
+        const double zn = z * zo * st->alpha_old / (alpha * st->beta_old * (zo - z) + zo * st->alpha_old * (1.0 + st->delta[i] * alpha));
+        st->znew[i] = zn;
+        st->ax[i] = alpha * zn / z;
+    }
+}
+// after the residual step: beta = c' / c, p_i = zeta_i' r + beta (zeta_i' / zeta_i)^2 p_i; then the state moves on
+__global__ void ms_beta_kernel(MsState* __restrict__ st, const double* __restrict__ sc, int slot_cn) {
+    if (threadIdx.x != 0) return;
+    const double cn = sc[slot_cn * MAXR];
+    const double beta = cn / st->cc;
+    for (int i = 0; i < st->n; ++i) {
+        const double ratio = st->znew[i] / st->zeta[i];
+        st->zr[i] = st->znew[i];
+        st->bp[i] = beta * ratio * ratio;
+        st->zeta_old[i] = st->zeta[i];
+        st->zeta[i] = st->znew[i];
+    }
+    st->alpha_old = st->alpha;
+    st->beta_old = beta;
+    st->cc = cn;
+}
+// |p_0|^2 of the new p_0 -> state (read by the next ms_alpha_kernel)
+__global__ void ms_p0_kernel(MsState* __restrict__ st, const double* __restrict__ sc, int slot) {
+    if (threadIdx.x == 0) st->p0n2 = sc[slot * MAXR];
+}
+
+// r -= alpha (z + s0 p_0) ; |r|^2
 template <typename R>
 __global__ void __launch_bounds__(256) ms_r_kernel(typename VB<R>::V* __restrict__ r, const typename VB<R>::V* __restrict__ z,
-                                                   const typename VB<R>::V* __restrict__ p0, R a, R as0, size_t nvec,
-                                                   double* __restrict__ partials) {
+                                                   const typename VB<R>::V* __restrict__ p0, const MsState* __restrict__ st,
+                                                   size_t nvec, double* __restrict__ partials) {
+    const R a = (R)st->alpha, as0 = (R)(st->alpha * st->s0);
     double acc = 0.0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
         typename VB<R>::V v = axpyv(-a, z[i], r[i]);
@@ -125,26 +162,24 @@ __global__ void __launch_bounds__(256) ms_r_kernel(typename VB<R>::V* __restrict
     if (threadIdx.x == 0) partials[blockIdx.x] = acc;
 }
 
-struct MsCoef {
-    int n;
-    double ax[16];    // x_i += ax_i p_i   (old p_i)
-    double zr[16];    // p_i  = zr_i r + bp_i p_i
-    double bp[16];
-};
-
-// for every shift i: x_i += ax_i p_i ; p_i = zr_i r + bp_i p_i ; |p_0|^2 of the new p_0.  r is read once.
+// for every shift i: x_i += ax_i p_i ; p_i = zr_i r + bp_i p_i ; |p_0|^2 of the new p_0.  r is read once.  A system whose
+// stopping test fired at an earlier iteration (conv[0] in [0, iter)) is left alone: the host runs one iteration ahead.
 template <typename R>
 __global__ void __launch_bounds__(256) ms_update_kernel(typename VB<R>::V* __restrict__ x, typename VB<R>::V* __restrict__ p,
-                                                        const typename VB<R>::V* __restrict__ r, size_t nvec, MsCoef c,
-                                                        double* __restrict__ partials) {
+                                                        const typename VB<R>::V* __restrict__ r, size_t nvec,
+                                                        const MsState* __restrict__ st, double* __restrict__ partials,
+                                                        const int* __restrict__ conv, int iter) {
+    const int cv = conv[0];
+    if (cv >= 0 && cv < iter) { if (threadIdx.x == 0) partials[blockIdx.x] = 0.0; return; }
+    const int n = st->n;
     double acc = 0.0;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < nvec; i += (size_t)gridDim.x * blockDim.x) {
         const typename VB<R>::V rv = r[i];
-        for (int k = 0; k < c.n; ++k) {
+        for (int k = 0; k < n; ++k) {
             const typename VB<R>::V pv = p[(size_t)k * nvec + i];
-            x[(size_t)k * nvec + i] = axpyv((R)c.ax[k], pv, x[(size_t)k * nvec + i]);
-            typename VB<R>::V pn = axpyv((R)c.bp[k], pv, typename VB<R>::V{});
-            pn = axpyv((R)c.zr[k], rv, pn);
+            x[(size_t)k * nvec + i] = axpyv((R)st->ax[k], pv, x[(size_t)k * nvec + i]);
+            typename VB<R>::V pn = axpyv((R)st->bp[k], pv, typename VB<R>::V{});
+            pn = axpyv((R)st->zr[k], rv, pn);
             p[(size_t)k * nvec + i] = pn;
             if (k == 0) acc += n2(pn);
         }
@@ -248,32 +283,36 @@ dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int p
     return DWF_OK;
 }
 
-// r -= a z + a s0 p0, |r|^2 -> scalars[slot]   (fp64 fields)
-dwf_status launch_ms_r(dwf_ctx* c, void* r, const void* z, const void* p0, double a, double as0, size_t nreal, int slot) {
+// r -= alpha (z + s0 p0), |r|^2 -> scalars[slot] with the stopping test of iteration `iter`   (fp64 fields)
+dwf_status launch_ms_r(dwf_ctx* c, void* r, const void* z, const void* p0, size_t nreal, int slot_d, int slot, int iter) {
     const size_t nvec = nreal / 2;
     const int grid = blas_grid(nvec);
     dwf_status st = ensure_partials(c, grid);
     if (st != DWF_OK) return st;
-    ms_r_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)r, (const double2*)z, (const double2*)p0, a, as0, nvec, c->partials);
-    c->launches++;
+    ms_alpha_kernel<<<1, 32, 0, c->stream>>>(c->ms_state, c->scalars, slot_d);
+    ms_r_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)r, (const double2*)z, (const double2*)p0, c->ms_state, nvec, c->partials);
+    c->launches += 2;
     DWF_CUDA_CHECK(c, cudaGetLastError());
-    return launch_reduce(c, grid, slot);
+    return launch_reduce(c, grid, slot, iter);
 }
 
-// all shifts at once (fields i at x + i*nreal, p + i*nreal); |p_0|^2 -> scalars[slot]
-dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t nreal, int n, const double* ax, const double* zr,
-                            const double* bp, int slot) {
+// all shifts at once (fields i at x + i*nreal, p + i*nreal); |p_0|^2 -> state
+dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t nreal, int slot_cn, int slot, int iter) {
     const size_t nvec = nreal / 2;
     const int grid = blas_grid(nvec);
     dwf_status st = ensure_partials(c, grid);
     if (st != DWF_OK) return st;
-    MsCoef co;
-    co.n = n;
-    for (int i = 0; i < 16; ++i) { co.ax[i] = i < n ? ax[i] : 0.0; co.zr[i] = i < n ? zr[i] : 0.0; co.bp[i] = i < n ? bp[i] : 0.0; }
-    ms_update_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)x, (double2*)p, (const double2*)r, nvec, co, c->partials);
+    ms_beta_kernel<<<1, 32, 0, c->stream>>>(c->ms_state, c->scalars, slot_cn);
+    ms_update_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)x, (double2*)p, (const double2*)r, nvec, c->ms_state, c->partials,
+                                                          c->cg_conv, iter);
+    c->launches += 2;
+    DWF_CUDA_CHECK(c, cudaGetLastError());
+    st = launch_reduce(c, grid, slot, 0);
+    if (st != DWF_OK) return st;
+    ms_p0_kernel<<<1, 32, 0, c->stream>>>(c->ms_state, c->scalars, slot);
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
-    return launch_reduce(c, grid, slot);
+    return DWF_OK;
 }
 
 dwf_status launch_lincomb3(dwf_ctx* c, void* out, const void* x, const void* y, const void* z, double a, double b, double cc,

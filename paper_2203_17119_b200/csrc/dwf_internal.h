@@ -49,6 +49,14 @@ enum Op5 { OP_A = 0, OP_ADAG, OP_MEE, OP_MEEDAG, OP_MEEINV, OP_MEEINVDAG,
            OP_MEEINVDAG_ADAG,  // Mee^-dag * A^dag      (middle of Mpc^dag)
            OP5_COUNT };
 
+// device-resident scalar state of the multishift CG (dwf_blas.cu): zeta recurrences of every shift, the base system's
+// alpha / beta / |r|^2 / |p_0|^2 and the coefficients the vector kernels read
+struct MsState {
+    int n;
+    double s0, cc, p0n2, alpha, alpha_old, beta_old;
+    double delta[16], zeta[16], zeta_old[16], znew[16], ax[16], zr[16], bp[16];
+};
+
 struct DevTables {           // device copies, [OP5_COUNT][2][Ls*Ls]
     double* d64 = nullptr;
     float* d32 = nullptr;
@@ -101,6 +109,7 @@ struct dwf_ctx {
     // workspace (allocated lazily, sized for half fields)
     void* ws64[10] = {};
     void* ws32[10] = {};
+    dwf::MsState* ms_state = nullptr;   // multishift CG: device-resident scalar recurrences
     void* ms_p = nullptr;        // multishift CG: search directions of all shifts
     size_t ms_p_bytes = 0;
     double* partials = nullptr;  // per-block reduction partials
@@ -193,9 +202,10 @@ dwf_status launch_xpay(dwf_ctx* c, void* p, const void* r, int prec, size_t nrea
 dwf_status launch_axpy(dwf_ctx* c, void* y, const void* x, double a, int prec, size_t nreal);  // y += a x
 dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int prec, size_t nreal);  // out = a - b
 dwf_status launch_add_f32_to_f64(dwf_ctx* c, void* x64, const void* e32, size_t unused);  // x += (double)e, half field
-dwf_status launch_ms_r(dwf_ctx* c, void* r, const void* z, const void* p0, double a, double as0, size_t nreal, int slot);
-dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t nreal, int n, const double* ax, const double* zr,
-                            const double* bp, int slot);
+// multishift CG: alpha / zeta recurrences from scalars[slot_d] and c->ms_state, then r -= alpha (z + s0 p_0), |r|^2 -> slot (+ test)
+dwf_status launch_ms_r(dwf_ctx* c, void* r, const void* z, const void* p0, size_t nreal, int slot_d, int slot, int iter);
+// beta and the update coefficients from scalars[slot_cn], then all shifts: x_i += .., p_i = ..; |p_0|^2 -> slot and state
+dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t nreal, int slot_cn, int slot, int iter);
 dwf_status launch_lincomb3(dwf_ctx* c, void* out, const void* x, const void* y, const void* z, double a, double b, double cc,
                            int prec, size_t nreal);   // out = a x + b y + cc z
 dwf_status ensure_partials(dwf_ctx* c, int n);
