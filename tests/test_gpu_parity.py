@@ -251,10 +251,10 @@ def test_multishift_cg_matches_oracle(case):
     from oracle.dwf_oracle import multishift_cg
     g, A = case.gpu, case.api
     # the oracle's multishift CG takes minutes to 1e-10 with four shifts on the larger lattices (every Ls = 12 / 16 one and the
-    # generic-Ls one): two shifts to 1e-6 there -- same kernels, same recurrences, fewer iterations
+    # generic-Ls one): two shifts to 1e-5 there -- same kernels, same recurrences, fewer iterations
     slow = int(np.prod(case.dims)) * case.Ls > 13000 or case.Ls == 5
     shifts = [0.0, 0.4] if slow else [0.0, 0.02, 0.4, 3.0]
-    tol = 1e-6 if slow else 1e-10
+    tol = 1e-5 if slow else 1e-10
     xs_ref, info_ref = multishift_cg(case.orc, case.odd, shifts, tol, 5000)
     xs, info, res, st = g.multishift_cg(g.pack(case.odd, A.F64, A.ODD), shifts, tol, 5000)
     assert st == A.OK and info_ref["converged"]
