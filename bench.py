@@ -306,11 +306,11 @@ def run_dwf(args, cfg):
     src32 = g.convert(b, A.F64, A.F32, A.ODD)
     out32 = g.new_native(A.F32, A.ODD)
     for _ in range(3):
-        g.chebyshev(src32, 0.0, 200.0, 2 * iters, A.F32, out=out32)
+        g.chebyshev(src32, 0.0, 5000.0, 2 * iters, A.F32, out=out32)
     g.set_option("time_dhop", 1)
     torch.cuda.synchronize()
     for _ in range(args.steps):
-        g.chebyshev(src32, 0.0, 200.0, 2 * iters, A.F32, out=out32)
+        g.chebyshev(src32, 0.0, 5000.0, 2 * iters, A.F32, out=out32)
     ms32, n32, by32 = g.get_option("dhop_ms"), g.get_option("dhop_timed"), g.get_option("dhop_bytes")
     g.set_option("time_dhop", 0)
     del src32, out32
