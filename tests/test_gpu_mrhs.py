@@ -20,6 +20,8 @@ CASES = {
     "ragged_ls5": dict(dims=(4, 6, 4, 8), Ls=5, par=MOEB, eps=0.5, nrhs=4),
     # 18-real links (unfused), six systems
     "g18": dict(dims=(4, 4, 4, 8), Ls=4, par=MOEB, eps=0.6, compress12=0, nrhs=6),
+    # the largest batch the ABI accepts, on the fused path
+    "max16": dict(dims=(4, 4, 4, 4), Ls=4, par=SHAM, eps=0.3, nrhs=16),
 }
 
 

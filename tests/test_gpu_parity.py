@@ -86,6 +86,8 @@ CASES = {
     "g18": dict(dims=(4, 4, 8, 8), Ls=8, par=MOEB, eps=0.7, compress12=0),
     # smallest legal lattice, Ls = 1
     "tiny": dict(dims=(2, 2, 2, 2), Ls=1, par=MOEB, eps=0.7),
+    # the largest fifth dimension the ABI accepts (Ls = 32: generic-Ls column kernels, 32 slices per tile in the TMA kernel)
+    "ls32": dict(dims=(4, 4, 4, 4), Ls=32, par=MOEB, eps=0.4, fused=True),
     # non-default tiles
     "tiles": dict(dims=(8, 8, 4, 8), Ls=4, par=MOEB, eps=0.7, tiles=(8, 2, 2, 4)),
     # the fused-epilogue Dhop kernels (4^4 tiles, Ls in {8, 12, 16}) -- c1, cut and cut2 above run them too -- and the
