@@ -247,16 +247,29 @@ def test_host_entry_points(case):
     assert np.sqrt(case.orc.norm2(case.full - case.orc.M(psi)) / case.orc.norm2(case.full)) < 1e-6
 
 
-def test_multishift_cg_matches_oracle(case):
+# the multishift kernels do not depend on which Dhop kernel runs underneath: one lattice per code path they do depend on
+# (fused / unfused Mpc, generic Ls, cut links, 18-real links, Ls = 1 and Ls = 32)
+MS_CASES = ["c1", "ragged", "ls5", "cut", "g18", "tiny", "fused12", "ls32"]
+
+
+@pytest.fixture(scope="module", params=MS_CASES)
+def ms_case(request, api, oracle_built):
+    c = Case(api, **CASES[request.param])
+    yield c
+    c.gpu.close()
+
+
+def test_multishift_cg_matches_oracle(ms_case):
     """NEXT-2 (eqs. 20-21): all shifted solutions of (Mpc^dag Mpc + sigma_i) x_i = b against the
     oracle's multishift CG, shared iteration count within +-2, true residuals recomputed by the oracle."""
+    case = ms_case
     from oracle.dwf_oracle import multishift_cg
     g, A = case.gpu, case.api
     # the oracle's multishift CG takes minutes to 1e-10 with four shifts on the larger lattices (every Ls = 12 / 16 one and the
-    # generic-Ls one): two shifts to 1e-5 there -- same kernels, same recurrences, fewer iterations
+    # generic-Ls one): two shifts to 1e-4 there -- same kernels, same recurrences, fewer iterations
     slow = int(np.prod(case.dims)) * case.Ls > 13000 or case.Ls == 5
     shifts = [0.0, 0.4] if slow else [0.0, 0.02, 0.4, 3.0]
-    tol = 1e-5 if slow else 1e-10
+    tol = 1e-4 if slow else 1e-10
     xs_ref, info_ref = multishift_cg(case.orc, case.odd, shifts, tol, 5000)
     xs, info, res, st = g.multishift_cg(g.pack(case.odd, A.F64, A.ODD), shifts, tol, 5000)
     assert st == A.OK and info_ref["converged"]
