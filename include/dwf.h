@@ -128,6 +128,30 @@ dwf_status dwf_mdagm(dwf_ctx* ctx, void* out_dev, const void* in_dev, dwf_prec p
 /* sum |v|^2 over a native field, accumulated in fp64 with a fixed reduction tree (deterministic) */
 dwf_status dwf_norm2(dwf_ctx* ctx, const void* v_dev, dwf_prec prec, dwf_parity parity, double* result_host);
 
+/* The same sum for callers that must not allocate device memory.  dwf_norm2 above, like every solver here, keeps its
+ * per-block partial sums in a buffer its context gets from cudaMalloc.  That rules the library out for programs that have
+ * handed the whole device to their own memory pool at start-up (lattice codes and tensor frameworks do: a library's
+ * cudaMalloc then fails or eats into the pool), for latency-critical paths that cannot take the device-wide synchronisation
+ * a cudaMalloc / cudaFree implies, and for plug-ins whose host forbids allocation in its callbacks.  This entry point needs
+ * no context and calls no cudaMalloc, cudaFree or allocating library routine: its partial sums go to a fixed 512 KiB array
+ * inside the library image (present on every GPU that loads the library, until the process exits).
+ *   v_dev       DEVICE pointer, 16-byte aligned, nreal reals of precision prec, any layout (a native or canonical field of
+ *               any parity, or any other array); read only.  nreal: a multiple of 2 (fp64) / 4 (fp32); 0 gives 0.0.
+ *   result_dev  DEVICE pointer to one double owned by the caller, 8-byte aligned; written by the last kernel enqueued.
+ *   cuda_stream cudaStream_t as void* (NULL = default stream).  Two kernels are enqueued, nothing is synchronised: read
+ *               *result_dev after ordering against that stream.  The device is the one current at the call.
+ *   errbuf      optional HOST buffer of errbuf_len bytes for a message when the status is not DWF_OK (may be NULL).
+ * Limit: nreal * sizeof(real) <= DWF_NORM2_STATIC_MAX_BYTES (4 GiB: one partial per 64 KiB of input, 65536 slots).  A larger
+ *   input returns DWF_EINVAL and enqueues nothing; so do null / misaligned pointers.  DWF_ECUDA: a runtime call failed.
+ * Sharing: all calls on one device use the same array.  Nothing in it has to be zero beforehand (a call writes every slot
+ *   it later reads), but calls that may overlap on the GPU - other streams, other threads - race on it: order them.
+ * First call on each device: looks up the array's device address once (cudaGetSymbolAddress) and caches it; make that call
+ *   outside any stream capture.  Accumulation in fp64 with a fixed tree that depends on nreal only: the same input gives
+ *   the same bits on every run and every GPU; it agrees with dwf_norm2 to rounding (a different, also fixed, tree). */
+#define DWF_NORM2_STATIC_MAX_BYTES 4294967296ull
+dwf_status dwf_norm2_static(const void* v_dev, size_t nreal, dwf_prec prec, double* result_dev, void* cuda_stream,
+                            char* errbuf, size_t errbuf_len);
+
 /* CG on Mpc^dag Mpc x = b (reading C8; mixed: C9).  x_dev: in = initial guess (use_guess != 0) else ignored,
  * out = solution; both fp64 native ODD fields.  tol is relative to |b|.  Restarts from the true residual
  * until |b - A x| <= tol |b|.  Returns DWF_ENOTCONV if max_iter is reached.  The stopping test is evaluated on the device

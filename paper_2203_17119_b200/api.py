@@ -30,7 +30,7 @@ SYMBOLS = [
     "dwf_mooee_inv", "dwf_m", "dwf_mpc", "dwf_mdagm", "dwf_norm2", "dwf_cg", "dwf_multishift_cg", "dwf_chebyshev", "dwf_domain_project", "dwf_boundary_op", "dwf_solve", "dwf_dhop_host",
     "dwf_mdagm_host", "dwf_cg_host", "dwf_solve_host", "dwf_launch_count", "dwf_last_error", "dwf_version",
     "dwf_mrhs_reserve", "dwf_mrhs_field_bytes", "dwf_mrhs_insert", "dwf_mrhs_extract", "dwf_dhop_mrhs", "dwf_mpc_mrhs",
-    "dwf_mdagm_mrhs", "dwf_cg_mrhs",
+    "dwf_mdagm_mrhs", "dwf_cg_mrhs", "dwf_norm2_static",
 ]
 
 
@@ -81,6 +81,7 @@ def load_library():
     lib.dwf_mpc.argtypes = [vp, vp, vp, ci, ci]
     lib.dwf_mdagm.argtypes = [vp, vp, vp, ci]
     lib.dwf_norm2.argtypes = [vp, vp, ci, ci, P(cd)]
+    lib.dwf_norm2_static.argtypes = [vp, ctypes.c_size_t, ci, vp, vp, ctypes.c_char_p, ctypes.c_size_t]
     lib.dwf_cg.argtypes = [vp, vp, vp, cd, ci, ci, ci, P(CgInfo)]
     lib.dwf_domain_project.argtypes = [vp, vp, vp, ci, ci]
     lib.dwf_boundary_op.argtypes = [vp, vp, vp, ci, cd, ci, ci, P(CgInfo)]
@@ -390,6 +391,33 @@ class Dwf:
         st = self._chk(self.lib.dwf_solve_host(self._h, self._hp(psi_host), self._hp(eta_host), tol, max_iter, mode,
                                                ctypes.byref(info)), allow=(ENOTCONV,))
         return psi_host, info.as_dict(), st
+
+
+NORM2_STATIC_MAX_BYTES = 1 << 32      # DWF_NORM2_STATIC_MAX_BYTES of include/dwf.h
+
+
+def norm2_static(v, out, prec=None, stream=None):
+    """dwf_norm2_static: sum |v|^2 of a CUDA tensor into the one-element fp64 CUDA tensor `out`, for callers whose device
+    memory is all spoken for.  Unlike Dwf.norm2 it needs no context and the library allocates nothing for it: the partial
+    sums go to a fixed 512 KiB array built into libdwf_b200.so, which is why `v` may hold at most NORM2_STATIC_MAX_BYTES
+    (4 GiB; DwfError otherwise).  `v`: contiguous real tensor (float64 / float32) on the current device, any layout.  Two
+    kernels are enqueued on `stream` (default: torch's current stream) and nothing waits for them: `out.item()` or a stream
+    synchronise gives the value.  Calls on one device share the array, so do not let two of them overlap on the GPU.  This
+    wrapper only marshals the arguments (it allocates nothing either; `out` is the caller's)."""
+    lib = load_library()
+    if not torch.cuda.is_available():
+        raise RuntimeError("paper_2203_17119_b200 needs a CUDA device (no CPU fallback)")
+    prec = (F64 if v.dtype == torch.float64 else F32) if prec is None else prec
+    assert v.is_cuda and v.is_contiguous() and v.dtype == _rdtype(prec)
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 1 and out.device == v.device
+    s = torch.cuda.current_stream(v.device).cuda_stream if stream is None else int(stream)
+    err = ctypes.create_string_buffer(256)
+    with torch.cuda.device(v.device):
+        st = lib.dwf_norm2_static(ctypes.c_void_p(v.data_ptr()), v.numel(), prec, ctypes.c_void_p(out.data_ptr()),
+                                  ctypes.c_void_p(s), err, len(err))
+    if st != OK:
+        raise DwfError(st, err.value.decode())
+    return out
 
 
 def from_config(cfg, **options) -> Dwf:

@@ -15,7 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libdwf_b200.so")
-SOURCES = ["dwf_api.cu", "dwf_dhop.cu", "dwf_dhop_pipe.cu", "dwf_dhop_tma.cu", "dwf_fived.cu", "dwf_blas.cu", "dwf_gauge.cu"]
+SOURCES = ["dwf_api.cu", "dwf_dhop.cu", "dwf_dhop_pipe.cu", "dwf_dhop_tma.cu", "dwf_fived.cu", "dwf_blas.cu", "dwf_gauge.cu",
+           "dwf_noalloc.cu"]
 # IEEE arithmetic on purpose: no --use_fast_math
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"]
