@@ -98,7 +98,12 @@ dwf_status dwf_set_stream(dwf_ctx* ctx, void* cuda_stream);
  * fp64 and fp32 (round to nearest) for both parities, optionally 2-row compressed.  When a Dirichlet cut is configured
  * the same copies are also kept WITHOUT the cut (used only inside dwf_boundary_op; every other operator sees the cut
  * links).  The native layout is opaque and precision-specific (fp64 and fp32 fields order the sites of a
- * tile differently): move data between precisions with dwf_convert, never by casting a native buffer. */
+ * tile differently): move data between precisions with dwf_convert, never by casting a native buffer.
+ * With "compress12" = 1 (the default) the third row of every link is rebuilt as conj(row0 x row1), which is the same
+ * operator only for SU(3) links: the call first measures max |row2 - conj(row0 x row1)| over all links and returns
+ * DWF_EINVAL (message with the measured defect) when it exceeds 1e-10, an absolute bound that fp64 SU(3) links meet and
+ * links that went through single precision (defect ~1e-7) do not; reunitarise those, or set "compress12" = 0 to keep all
+ * 18 reals.  Also allocates the solver workspace (10 half fields per precision): DWF_ENOMEM if that fails. */
 dwf_status dwf_set_gauge(dwf_ctx* ctx, const void* U_dev_canonical_f64);
 
 /* Bytes of a native field of the given precision and parity (DWF_FULL = 2 x half). */
@@ -154,7 +159,8 @@ dwf_status dwf_norm2_static(const void* v_dev, size_t nreal, dwf_prec prec, doub
 
 /* CG on Mpc^dag Mpc x = b (reading C8; mixed: C9).  x_dev: in = initial guess (use_guess != 0) else ignored,
  * out = solution; both fp64 native ODD fields.  tol is relative to |b|.  Restarts from the true residual
- * until |b - A x| <= tol |b|.  Returns DWF_ENOTCONV if max_iter is reached.  The stopping test is evaluated on the device
+ * until |b - A x| <= tol |b|.  Returns DWF_ENOTCONV if max_iter is reached: max_iter bounds iters_total, the iterations
+ * counted over all restarts / inner solves (for a batch: of the system that needed most).  The stopping test is evaluated on the device
  * and the host enqueues one iteration ahead of the residual it has read: info->launches may include the kernels of one
  * iteration past the last counted one, which leave x untouched (x is exactly the iterate of iteration iters_total). */
 dwf_status dwf_cg(dwf_ctx* ctx, void* x_dev, const void* b_dev, double tol, int max_iter, dwf_cg_mode mode,
@@ -201,8 +207,8 @@ dwf_status dwf_chebyshev(dwf_ctx* ctx, void* out_dev, const void* in_dev, double
  * dwf_domain_project: out = P in on FULL native fields (out may alias in), which = 0: P_Omega, 1: P_Omegabar, 2: the
  *   boundary projector P_dbar of eq. 8, found by mask-and-shift: sites of Omega with a cut
  *   link, times (1 +- gamma_mu)/2 for Shamir sites on one cut face, times 1 otherwise (reading in DESIGN.md section 2).
- * dwf_boundary_op: FULL fp64 native fields, out != in.  inverse = 0: R phi = P phi - P D_O^-1 D_d D_Ob^-1 D_dbar phi (eq. 13,
- *   PAPER.md:107-109; two Dirichlet solves); inverse != 0: R^-1 phi = P phi - P D^-1 D_dbar_hat phi (eq. 14, PAPER.md:111-113;
+ * dwf_boundary_op: FULL fp64 native fields, out != in.  inverse = 0: R phi = P phi - P D_O^-1 D_d D_Ob^-1 D_dbar phi (eqs. 9-10,
+ *   PAPER.md:93-97; two Dirichlet solves); inverse != 0: R^-1 phi = P phi - P D^-1 D_dbar_hat phi (eqs. 13-14, PAPER.md:109-111;
  *   one solve with the uncut operator).  Solves as dwf_solve (tol, max_iter, mode); info->iters_total sums them,
  *   info->resid_full is the worst |eta - M psi|/|eta|.  Synchronises. */
 dwf_status dwf_domain_project(dwf_ctx* ctx, void* out_dev, const void* in_dev, int which, dwf_prec prec);

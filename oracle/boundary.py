@@ -17,8 +17,8 @@ face the projector is the boundary mask times (1 +- gamma_mu)/2 -- the minimal o
 identity in spin and s, the smallest coordinate projector that contains the minimal one.  Eqs. 13-14 hold for any
 projector with D_dbar P = D_dbar (R R^-1 = P follows from X P = X, X = D_O^-1 D_d D_Ob^-1 D_dbar).
 
-    R    phi = P phi - P D_O^-1 D_d D_Ob^-1 D_dbar phi        (eq. 13)
-    R^-1 phi = P phi - P D^-1 D_dbar_hat phi                  (eq. 14)
+    R    phi = P phi - P D_O^-1 D_d D_Ob^-1 D_dbar phi        (eqs. 9-10)
+    R^-1 phi = P phi - P D^-1 D_dbar_hat phi                  (eqs. 13-14)
 """
 from __future__ import annotations
 
@@ -89,7 +89,7 @@ class Boundary:
         """P_O D P_Ob psi."""
         return self.P_domain(self.full.M(self.P_domain(psi, False)), True)
 
-    # ---- eqs. 13, 14 -------------------------------------------------------------------------------------------
+    # ---- eqs. 13-14 (R^-1, PAPER.md:109-111) and eqs. 9-10 (R, PAPER.md:93-97) -------------------------------------------------------------------------------------------
     def R_inv(self, phi, tol=1e-12, max_iter=20000):
         u = self.D_dbar_hat(phi)
         v, info = solve_redblack(self.full, u, tol, max_iter)

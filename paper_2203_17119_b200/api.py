@@ -331,7 +331,7 @@ class Dwf:
         return out
 
     def boundary_op(self, phi, inverse, tol, max_iter, mode=CG_F64, out=None):
-        """R phi (inverse False, eq. 13) or R^-1 phi (inverse True, eq. 14); FULL fp64 native fields."""
+        """R phi (inverse False, eqs. 9-10) or R^-1 phi (inverse True, eqs. 13-14); FULL fp64 native fields."""
         out = self.new_native(F64, FULL) if out is None else out
         info = CgInfo()
         st = self._chk(self.lib.dwf_boundary_op(self._h, self._p(out), self._p(phi), int(bool(inverse)), tol, max_iter, mode,

@@ -35,10 +35,7 @@ def _deps_mtime() -> float:
 
 
 def _flags() -> list:
-    """DWF_PROBE=1 in the environment compiles the measurement knobs in (tile order, grid size, halo skipping ...:
-    dwf_set_option keys the product build rejects); the product build is the one without it."""
-    extra = os.environ.get("DWF_NVCC_EXTRA", "").split()           # experiments only, e.g. DWF_NVCC_EXTRA=-DDWF_REMAT_N=2
-    return NVCC_FLAGS + (["-DDWF_PROBE"] if os.environ.get("DWF_PROBE", "0") not in ("", "0") else []) + extra
+    return NVCC_FLAGS
 
 
 def _stamp_ok() -> bool:

@@ -1,9 +1,10 @@
 // C-ABI entry points (include/dwf.h), operator compositions and the CG drivers.
 //
 // Compositions (reading C5/C6; Meooe = -1/2 Dhop A, Mpc = Moo - Moe Mee^-1 Meo on odd sites):
-//   Mpc x     = Moo x - 1/4 Dhop_o [A Mee^-1] Dhop_e [A] x                 (5 kernels)
+//   Mpc x     = Moo x - 1/4 Dhop_o [A Mee^-1] Dhop_e [A] x                 (5 kernels; 4 on the fused path, where the
+//                                                                            second Dhop adds Moo x in its epilogue)
 //   Mpc^dag x = Moo^dag x - 1/4 A^dag Dhop^dag_o [Mee^-dag A^dag] Dhop^dag_e x   (4 kernels)
-// where [..] are single fused 5-D table kernels and the final 5-D kernel also adds the Moo term and,
+// where [..] are single fused 5-D table kernels and the final kernel also adds the Moo term and,
 // inside CG, accumulates |Mpc p|^2.
 #include <chrono>
 #include <cmath>
@@ -17,9 +18,13 @@ namespace {
 
 const int NWS = 10;
 
-// The solver workspace (NWS half fields per precision) is allocated once, at dwf_set_gauge: no operator, dwf_cg or
-// dwf_solve call allocates device memory ("ctx owns ... CG workspace; no allocation inside dwf_cg").
-// The batched (multi right-hand side) calls have their own set, sized by dwf_mrhs_reserve (or by the first batched call).
+// The solver workspace (NWS half fields per precision, both precisions, whatever the caller goes on to use) is allocated
+// once, at dwf_set_gauge, so that the vectors of dwf_cg / dwf_solve are never allocated inside a solve ("ctx owns
+// ... CG workspace").  What is still allocated on first use, inside the first call that needs it, and then kept: the
+// reduction partials (ensure_partials: a few KB, grows only when a larger grid or batch first appears), the multishift
+// state and its nshift direction fields (dwf_multishift_cg), the two FULL fields of dwf_boundary_op, the device staging
+// buffers of the *_host calls, and the batched workspace (dwf_mrhs_reserve, or the first batched call with a larger nrhs:
+// NWSM fields of nrhs systems in both precisions).  dwf_norm2_static (dwf_noalloc.cu) is the one call that allocates nothing.
 dwf_status ws_alloc_all(dwf_ctx* c) {
     for (int prec = 0; prec < 2; ++prec) {
         void** arr = (prec == DWF_F64) ? c->ws64 : c->ws32;
@@ -159,8 +164,9 @@ dwf_status m_apply(dwf_ctx* c, void* out, const void* in, int dagger, int prec) 
 // ---- CG on A = Mpc^dag Mpc for the c->nrhs_cur systems of a (batched) field (readings C8, C9) ------------------------
 // The stopping test lives on the device (reduce_partials_kernel: cg_conv[j] = first iteration with |r_j|^2 <= cg_target[j])
 // and the host enqueues iteration k + 1 before it has read the residual of iteration k: the GPU never waits for the host.
-// Iteration k + 1 of a system that stopped at k only touches work vectors (cg_xp / cg_update leave x and p alone), so the
-// solution is the iterate of iteration k exactly, and the iteration count reported is k -- as in the oracle's loop.
+// Iteration k + 1 of a system that stopped at k only touches work vectors (cg_xp and cg_update leave x alone; the fused
+// path also freezes p and r and zeroes the system's Dhop chain, the unfused path simply lets the recurrence of r and p run
+// on), so the solution is the iterate of iteration k exactly, and the iteration count reported is k -- as in the oracle's loop.
 struct CgRun {
     int n;                       // systems
     double target[MAXR];         // tol^2 |b|^2 (or the inner target), per system
@@ -303,7 +309,7 @@ dwf_status cg_f64(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, 
     CgRun run;
     run.n = N;
     for (int j = 0; j < N; ++j) run.target[j] = tol * tol * bn2[j];
-    int iters[MAXR] = {}, restarts = 0, launched = 0;
+    int iters[MAXR] = {}, restarts = 0, most = 0;       // most: the largest iteration count of any system so far
     double rt[MAXR];
     bool conv = false;
     for (;;) {
@@ -313,10 +319,12 @@ dwf_status cg_f64(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, 
             DWF_CUDA_CHECK(c, cudaMemcpyAsync(r, b, hb, cudaMemcpyDeviceToDevice, c->stream));
             for (int j = 0; j < N; ++j) run.c[j] = bn2[j];
         }
-        DWF_TRY(cg_iterate(c, DWF_F64, x, r, max_iter - launched, run));
-        launched += run.launched;
+        // the budget is spent by COUNTED iterations (as in the oracle's loop), not by enqueued ones: the iteration the host
+        // runs ahead of the stopping test costs nothing
+        DWF_TRY(cg_iterate(c, DWF_F64, x, r, max_iter - most, run));
         for (int j = 0; j < N; ++j) {
             iters[j] += run.iters[j];
+            most = iters[j] > most ? iters[j] : most;
             info[j].resid_iter = bn2[j] > 0 ? std::sqrt(run.c[j] / bn2[j]) : 0.0;
         }
         void* tr;
@@ -328,10 +336,7 @@ dwf_status cg_f64(dwf_ctx* c, void* x, const void* b, double tol, int max_iter, 
             rt[j] = bn2[j] > 0 ? std::sqrt(tn2[j] / bn2[j]) : 0.0;
             conv = conv && rt[j] <= tol;
         }
-        if (conv) break;
-        int most = 0;
-        for (int j = 0; j < N; ++j) most = iters[j] > most ? iters[j] : most;
-        if (most >= max_iter || launched >= max_iter) break;
+        if (conv || most >= max_iter) break;
         ++restarts;
     }
     for (int j = 0; j < N; ++j) {
@@ -357,7 +362,7 @@ dwf_status cg_mixed(dwf_ctx* c, void* x, const void* b, double tol, int max_iter
     bool any = false;
     for (int j = 0; j < N; ++j) any = any || bn2[j] != 0.0;
     if (!any) return DWF_OK;
-    int iters[MAXR] = {}, restarts = 0, launched = 0, outer[MAXR] = {};
+    int iters[MAXR] = {}, restarts = 0, most = 0, outer[MAXR] = {};      // most: as in cg_f64, counted iterations
     double rt[MAXR];
     bool conv = false;
     for (;;) {
@@ -368,7 +373,7 @@ dwf_status cg_mixed(dwf_ctx* c, void* x, const void* b, double tol, int max_iter
             rt[j] = bn2[j] > 0 ? std::sqrt(rn2[j] / bn2[j]) : 0.0;
             conv = conv && rt[j] <= tol;
         }
-        if (conv || restarts >= c->max_restarts || launched >= max_iter) break;
+        if (conv || restarts >= c->max_restarts || most >= max_iter) break;
         DWF_TRY(launch_convert(c, r32, DWF_F32, r, DWF_F64, 1));
         CgRun run;
         run.n = N;
@@ -382,10 +387,10 @@ dwf_status cg_mixed(dwf_ctx* c, void* x, const void* b, double tol, int max_iter
             run.target[j] = delta * delta * r32n2[j];
             ++outer[j];
         }
-        DWF_TRY(cg_iterate(c, DWF_F32, e32, r32, max_iter - launched, run));
-        launched += run.launched;
+        DWF_TRY(cg_iterate(c, DWF_F32, e32, r32, max_iter - most, run));
         for (int j = 0; j < N; ++j) {
             iters[j] += run.iters[j];
+            most = iters[j] > most ? iters[j] : most;
             if (r32n2[j] > 0 && rt[j] > tol) info[j].resid_iter = std::sqrt(run.c[j] / r32n2[j]);
         }
         DWF_TRY(launch_add_f32_to_f64(c, x, e32, 0));
@@ -463,6 +468,10 @@ dwf_status dwf_create(dwf_ctx** out, const int dims[4], int Ls, double M5, doubl
     c->g.Ls = Ls;
     c->g.antiperiodic_t = 1;
     cudaGetDevice(&c->device);
+    if (cudaDeviceGetAttribute(&c->num_sms, cudaDevAttrMultiProcessorCount, c->device) != cudaSuccess || c->num_sms < 1) {
+        cudaGetLastError();
+        c->num_sms = 148;
+    }
     c->M5 = M5; c->mf = mf; c->b5 = b5; c->c5 = c5;
     choose_tiles(c);
     build_tables(c);
@@ -565,19 +574,6 @@ dwf_status dwf_set_option(dwf_ctx* c, const char* key, double val) {
     else if (k == "dhop_kernel") c->dhop_kernel = (int)val;
     else if (k == "fuse") c->fuse = (val != 0.0);
     else if (k == "dhop_dynamic") { if (val < 0 || val > 1) return DWF_EINVAL; c->dhop_dynamic = (int)val; }
-#ifdef DWF_PROBE
-    // measurement knobs of the probe build (python -m paper_2203_17119_b200.build with DWF_PROBE=1); not part of the ABI
-    else if (k == "dhop_sc") { if (val < 0 || val > 4) return DWF_EINVAL; c->dhop_sc = (int)val; }
-    else if (k == "dhop_loop_s") c->dhop_loop_s = (val != 0.0);
-    else if (k == "dhop_grid") { if (val < 0) return DWF_EINVAL; c->dhop_grid = (int)val; }
-    else if (k == "dhop_order" || k == "dhop_order_axes") {
-        if (val < 0 || val > 9999) return DWF_EINVAL;
-        (k == "dhop_order" ? c->dhop_order : c->dhop_order_axes) = (int)val;
-        if (c->gauge_set) DWF_TRY(tma_state_build(c));
-    }
-    else if (k == "dhop_skip") c->dhop_skip = (int)val;
-    else if (k == "dhop_nst") { if (val != 2 && val != 3) return DWF_EINVAL; c->dhop_nst = (int)val; }
-#endif
     else if (k == "time_dhop") {       // (re)start per-launch event timing of the Dhop kernel
         DWF_TRY(dhop_timing_flush(c));
         c->time_dhop = (val != 0.0);
@@ -997,7 +993,7 @@ dwf_status dwf_solve(dwf_ctx* c, void* psi, const void* eta, double tol, int max
     dwf_cg_info local;
     if (!info) info = &local;
     memset(info, 0, sizeof(*info));
-    if (!psi || !eta || psi == eta || tol <= 0.0) { c->err = "solve: bad arguments"; return DWF_EINVAL; }
+    if (!psi || !eta || psi == eta || tol <= 0.0 || max_iter < 0) { c->err = "solve: bad arguments"; return DWF_EINVAL; }
     const long long l0 = c->launches;
     const double t0 = now_s();
     const int P = DWF_F64;
@@ -1093,7 +1089,7 @@ dwf_status dwf_boundary_op(dwf_ctx* c, void* out, const void* in, int inverse, d
     dwf_cg_info local;
     if (!info) info = &local;
     memset(info, 0, sizeof(*info));
-    if (!out || !in || out == in || tol <= 0.0) { c->err = "boundary_op: bad arguments"; return DWF_EINVAL; }
+    if (!out || !in || out == in || tol <= 0.0 || max_iter < 0) { c->err = "boundary_op: bad arguments"; return DWF_EINVAL; }
     DWF_TRY(boundary_geometry_ok(c));
     const double t0 = now_s();
     const long long l0 = c->launches;
@@ -1113,7 +1109,7 @@ dwf_status dwf_boundary_op(dwf_ctx* c, void* out, const void* in, int inverse, d
     double rfull = 0.0;
     DWF_TRY(boundary_block(c, u, in, v, 0, 1));                         // u = D_dbar_hat phi            (on Omegabar)
     if (inverse) {
-        select_links(c, true);                                          // v = D^-1 u                    (eq. 14)
+        select_links(c, true);                                          // v = D^-1 u                    (eq. 13)
         st = dwf_solve(c, v, u, tol, max_iter, mode, &si);
         select_links(c, false);
         if (st != DWF_OK && st != DWF_ENOTCONV) return st;
@@ -1125,7 +1121,7 @@ dwf_status dwf_boundary_op(dwf_ctx* c, void* out, const void* in, int inverse, d
         if (st != DWF_OK) worst = st;
         iters += si.iters_total; rfull = si.resid_full;
         DWF_TRY(boundary_block(c, u, v, out, 1, 0));                    // u = D_d_hat v                 (on Omega; out as scratch)
-        st = dwf_solve(c, v, u, tol, max_iter, mode, &si);              // v = D_O^-1 u                  (eq. 13)
+        st = dwf_solve(c, v, u, tol, max_iter, mode, &si);              // v = D_O^-1 u                  (eq. 9)
         if (st != DWF_OK && st != DWF_ENOTCONV) return st;
         if (st != DWF_OK) worst = st;
         iters += si.iters_total; rfull = std::fmax(rfull, si.resid_full);

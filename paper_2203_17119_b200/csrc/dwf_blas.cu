@@ -200,9 +200,9 @@ __global__ void __launch_bounds__(256) lincomb3_kernel(typename VB<R>::V* out, c
     }
 }
 
-static inline int blas_grid(size_t nvec) {
+static inline int blas_grid(const dwf_ctx* c, size_t nvec) {
     size_t want = (nvec + 255) / 256;
-    size_t cap = 148 * 8;                    // 8 CTAs of 256 threads per SM, one wave
+    size_t cap = (size_t)c->num_sms * 8;     // 8 CTAs of 256 threads per SM, one wave
     return (int)(want < cap ? (want ? want : 1) : cap);
 }
 
@@ -215,7 +215,7 @@ static inline unsigned tile_chunk(const dwf_ctx* c, int prec) { return (unsigned
 // nreal: reals of ONE system; with c->nrhs_cur > 1 the field is batched and every system gets its own norm
 dwf_status launch_norm2(dwf_ctx* c, const void* v, int prec, size_t nreal, int slot) {
     const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
-    const int gridx = blas_grid(nvec);
+    const int gridx = blas_grid(c, nvec);
     const dim3 grid(gridx, c->nrhs_cur);
     const unsigned chunk = tile_chunk(c, prec);
     dwf_status st = ensure_partials(c, gridx);
@@ -230,7 +230,7 @@ dwf_status launch_norm2(dwf_ctx* c, const void* v, int prec, size_t nreal, int s
 dwf_status launch_cg_update(dwf_ctx* c, void* x, void* r, const void* p, const void* z, int prec, size_t nreal,
                             int slot_c, int slot_d, int slot_cn, int iter) {
     const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
-    const int gridx = blas_grid(nvec);
+    const int gridx = blas_grid(c, nvec);
     const dim3 grid(gridx, c->nrhs_cur);
     const unsigned chunk = tile_chunk(c, prec);
     dwf_status st = ensure_partials(c, gridx);
@@ -249,7 +249,7 @@ dwf_status launch_cg_update(dwf_ctx* c, void* x, void* r, const void* p, const v
 
 dwf_status launch_xpay(dwf_ctx* c, void* p, const void* r, int prec, size_t nreal, int slot_cn, int slot_c) {
     const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4);
-    const dim3 grid(blas_grid(nvec), c->nrhs_cur);
+    const dim3 grid(blas_grid(c, nvec), c->nrhs_cur);
     const unsigned chunk = tile_chunk(c, prec);
     DWF_BLAS_DISPATCH(prec,
                       (xpay_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)p, (const float4*)r, nvec, chunk, c->scalars,
@@ -264,7 +264,7 @@ dwf_status launch_xpay(dwf_ctx* c, void* p, const void* r, int prec, size_t nrea
 // elementwise kernels: nreal reals per system, all c->nrhs_cur systems of a batched field at once
 dwf_status launch_axpy(dwf_ctx* c, void* y, const void* x, double a, int prec, size_t nreal) {
     const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4) * c->nrhs_cur;
-    const int grid = blas_grid(nvec);
+    const int grid = blas_grid(c, nvec);
     DWF_BLAS_DISPATCH(prec, (axpy_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)y, (const float4*)x, (float)a, nvec)),
                       (axpy_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)y, (const double2*)x, a, nvec)));
     c->launches++;
@@ -274,7 +274,7 @@ dwf_status launch_axpy(dwf_ctx* c, void* y, const void* x, double a, int prec, s
 
 dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int prec, size_t nreal) {
     const size_t nvec = nreal / (prec == DWF_F64 ? 2 : 4) * c->nrhs_cur;
-    const int grid = blas_grid(nvec);
+    const int grid = blas_grid(c, nvec);
     DWF_BLAS_DISPATCH(prec,
                       (sub_kernel<float><<<grid, 256, 0, c->stream>>>((float4*)out, (const float4*)a, (const float4*)b, nvec)),
                       (sub_kernel<double><<<grid, 256, 0, c->stream>>>((double2*)out, (const double2*)a, (const double2*)b, nvec)));
@@ -286,7 +286,7 @@ dwf_status launch_sub(dwf_ctx* c, void* out, const void* a, const void* b, int p
 // r -= alpha (z + s0 p0), |r|^2 -> scalars[slot] with the stopping test of iteration `iter`   (fp64 fields)
 dwf_status launch_ms_r(dwf_ctx* c, void* r, const void* z, const void* p0, size_t nreal, int slot_d, int slot, int iter) {
     const size_t nvec = nreal / 2;
-    const int grid = blas_grid(nvec);
+    const int grid = blas_grid(c, nvec);
     dwf_status st = ensure_partials(c, grid);
     if (st != DWF_OK) return st;
     ms_alpha_kernel<<<1, 32, 0, c->stream>>>(c->ms_state, c->scalars, slot_d);
@@ -299,7 +299,7 @@ dwf_status launch_ms_r(dwf_ctx* c, void* r, const void* z, const void* p0, size_
 // all shifts at once (fields i at x + i*nreal, p + i*nreal); |p_0|^2 -> state
 dwf_status launch_ms_update(dwf_ctx* c, void* x, void* p, const void* r, size_t nreal, int slot_cn, int slot, int iter) {
     const size_t nvec = nreal / 2;
-    const int grid = blas_grid(nvec);
+    const int grid = blas_grid(c, nvec);
     dwf_status st = ensure_partials(c, grid);
     if (st != DWF_OK) return st;
     ms_beta_kernel<<<1, 32, 0, c->stream>>>(c->ms_state, c->scalars, slot_cn);
@@ -319,11 +319,11 @@ dwf_status launch_lincomb3(dwf_ctx* c, void* out, const void* x, const void* y, 
                            int prec, size_t nreal) {
     if (prec == DWF_F64) {
         const size_t nvec = nreal / 2;
-        lincomb3_kernel<double><<<blas_grid(nvec), 256, 0, c->stream>>>((double2*)out, (const double2*)x, (const double2*)y,
+        lincomb3_kernel<double><<<blas_grid(c, nvec), 256, 0, c->stream>>>((double2*)out, (const double2*)x, (const double2*)y,
                                                                         (const double2*)z, a, b, cc, nvec);
     } else {
         const size_t nvec = nreal / 4;
-        lincomb3_kernel<float><<<blas_grid(nvec), 256, 0, c->stream>>>((float4*)out, (const float4*)x, (const float4*)y,
+        lincomb3_kernel<float><<<blas_grid(c, nvec), 256, 0, c->stream>>>((float4*)out, (const float4*)x, (const float4*)y,
                                                                        (const float4*)z, (float)a, (float)b, (float)cc, nvec);
     }
     c->launches++;

@@ -110,7 +110,7 @@ static dwf_status launch_t(dwf_ctx* c, void* out, const void* in, const void* W,
     const int nchunks = (g.Ls + SC - 1) / SC;
     int block = 128;
     if (g.TS < block) block = ((g.TS + 31) / 32) * 32;
-    dim3 grid((g.Vh + block - 1) / block, c->dhop_loop_s ? 1 : nchunks);
+    dim3 grid((g.Vh + block - 1) / block, nchunks);
     if (dagger)
         dhop_kernel<R, SC, NG, true><<<grid, block, 0, c->stream>>>(g, (const V*)in, (V*)out, (const V*)W, out_parity, nchunks);
     else
@@ -127,7 +127,7 @@ static dwf_status launch_sc(dwf_ctx* c, void* out, const void* in, const void* W
         case 2: return launch_t<R, 2, NG>(c, out, in, W, out_parity, dagger);
         case 3: return launch_t<R, 3, NG>(c, out, in, W, out_parity, dagger);
         case 4: return launch_t<R, 4, NG>(c, out, in, W, out_parity, dagger);
-        default: c->err = "dhop_sc must be 1..4"; return DWF_EINVAL;
+        default: c->err = "dhop: slices per thread must be 1..4"; return DWF_EINVAL;
     }
 }
 
@@ -193,8 +193,7 @@ static dwf_status launch_dhop_untimed(dwf_ctx* c, void* out, const void* in, int
         if (st != DWF_OK || handled) return st;
     }
     const void* W = (prec == DWF_F64) ? c->W64[out_parity] : c->W32[out_parity];
-    int sc = c->dhop_sc;
-    if (sc <= 0) sc = (prec == DWF_F64) ? 2 : 4;
+    const int sc = (prec == DWF_F64) ? 2 : 4;       // s slices per thread
     if (prec == DWF_F64)
         return c->compress12 ? launch_sc<double, 12>(c, out, in, W, out_parity, dagger, sc)
                              : launch_sc<double, 18>(c, out, in, W, out_parity, dagger, sc);

@@ -1,4 +1,5 @@
-// Dhop, pipelined tile kernel (the fast path; dwf_dhop.cu keeps the shape-generic kernel).
+// Dhop, cp.async-pipelined tile kernel: the fallback for tile shapes and link formats the TMA kernel (dwf_dhop_tma.cu, the
+// fast path on 4^4 tiles with 2-row links) does not take; dwf_dhop.cu keeps the shape-generic kernel.
 //
 // One CTA owns one native tile (TS output sites of one parity) for ALL Ls slices:
 //   * every thread keeps its links in REGISTERS for the whole s loop (third row rebuilt once, the
@@ -353,12 +354,10 @@ dwf_status launch_dhop_pipe(dwf_ctx* c, void* out, const void* in, int out_parit
     a.slot_lane = c->pipe_slot_lane[pr] + (size_t)out_parity * c->pipe_nslot;
     a.out_parity = out_parity; a.dagger = dagger;
     const int TS = g.TS, NS = c->pipe_nslot;
-    const int nst = c->dhop_nst;
 #define DWF_PIPE_CASE(TSV, NSV)                                                                          \
     if (TS == TSV && NS == NSV) {                                                                        \
         *handled = true;                                                                                 \
         if (prec == DWF_F64) return launch_pipe_ng<double, 2, TSV, NSV, (3 * 12 * NSV * 16 <= 232448 ? 3 : 2)>(c, a); \
-        if (nst == 2) return launch_pipe_ng<float, 1, TSV, NSV, 2>(c, a);                                \
         return launch_pipe_ng<float, 1, TSV, NSV, 3>(c, a);                                              \
     }
     DWF_PIPE_CASE(128, 384)   // 4x4x4x4

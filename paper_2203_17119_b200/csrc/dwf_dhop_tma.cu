@@ -304,7 +304,7 @@ dwf_status tma_state_build(dwf_ctx* c) {
         std::vector<uint16_t> off(t64.off);
         off.insert(off.end(), t32.off.begin(), t32.off.end());
         const std::vector<uint16_t>& gdst = t64.gdst;
-        std::vector<uint32_t> order = build_order(g, c->dhop_order, c->dhop_order_axes);
+        std::vector<uint32_t> order = build_order(g, 0, 0);
         DWF_CUDA_CHECK(c, cudaMalloc(&s->off, off.size() * sizeof(uint16_t)));
         DWF_CUDA_CHECK(c, cudaMalloc(&s->xsrc, t32.xsrc.size()));
         DWF_CUDA_CHECK(c, cudaMalloc(&s->xdst, t32.xdst.size() * sizeof(uint16_t)));
@@ -523,14 +523,6 @@ __device__ __forceinline__ double vnorm2(const double2& a) { return a.x * a.x + 
 __device__ __forceinline__ float4 ldcs_v(const float4* p) { return __ldcs(p); }
 __device__ __forceinline__ double2 ldcs_v(const double2* p) { return __ldcs(p); }
 
-// halo regions the producer does not load: a traffic-attribution aid of the probe build only (results are then wrong);
-// the product build compiles every test on it away
-#ifdef DWF_PROBE
-#define SKIPM (a.skip)
-#else
-#define SKIPM 0
-#endif
-
 struct TmaArgs {
     Geom g;
     const void* in;
@@ -544,7 +536,6 @@ struct TmaArgs {
     const uint32_t* order;    // [ntiles]
     int* counters;            // [3] queue / done / round-arrival counters
     EpiArgs epi;
-    int skip;                 // debug: bit r set = do not load halo region r (4..11); results are then wrong, traffic only
     int mode;                 // 0: static round-robin, 1: global in-order queue
     int dagger;
 };
@@ -645,28 +636,27 @@ dhop_tma_kernel(const TmaArgs a, const __grid_constant__ CUtensorMap map_slab, c
                     // later (issued a whole tile ahead they were evicted again before use and fetched twice)
                     if (s == Ls - 1 && tile_next >= 0)
                         l2_prefetch_bulk(reinterpret_cast<const V*>(a.W) + (size_t)tile_next * 8 * KG * TSV, 8 * KG * TSV * 16);
-                    const int nskip = __popc(SKIPM & (GATHER_Y ? 0x0f0 : 0x3f0));
-                    mbar_arrive_expect_tx(full, (NTMA - nskip) * REGION_BYTES);
+                    mbar_arrive_expect_tx(full, NTMA * REGION_BYTES);
                     const int row_own = (tile * Ls + s) * K;
 #pragma unroll
                     for (int tt = 0; tt < 4; ++tt) tma_load_3d(base + tt * REGION_BYTES, &map_slab, 0, tt, row_own, full);
-                    if (!(SKIPM & 0x010)) tma_load_3d(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full);
-                    if (!(SKIPM & 0x020)) tma_load_3d(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full);
-                    if (!(SKIPM & 0x040)) tma_load_4d(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full);
-                    if (!(SKIPM & 0x080)) tma_load_4d(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full);
+                    tma_load_3d(base + 4 * REGION_BYTES, &map_slab, 0, 0, (nt[6] * Ls + s) * K, full);
+                    tma_load_3d(base + 5 * REGION_BYTES, &map_slab, 0, 3, (nt[7] * Ls + s) * K, full);
+                    tma_load_4d(base + 6 * REGION_BYTES, &map_z, 0, 0, 0, (nt[4] * Ls + s) * K, full);
+                    tma_load_4d(base + 7 * REGION_BYTES, &map_z, 0, 3, 0, (nt[5] * Ls + s) * K, full);
                     if (!GATHER_Y) {
-                        if (!(SKIPM & 0x100)) tma_load_4d(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full);
-                        if (!(SKIPM & 0x200)) tma_load_4d(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full);
+                        tma_load_4d(base + 8 * REGION_BYTES, &map_y, 0, 0, 0, (nt[2] * Ls + s) * K, full);
+                        tma_load_4d(base + 9 * REGION_BYTES, &map_y, 0, 3, 0, (nt[3] * Ls + s) * K, full);
                     }
                 }
                 const V* src = in + (size_t)s * (K * TSV);
 #pragma unroll
                 for (int k = 0; k < K; ++k) {
-                    if (!(SKIPM & 0x400)) cp_async16_tma(base + gd0 + k * 512, src + i0 + k * TSV);
-                    if (!(SKIPM & 0x800)) cp_async16_tma(base + gd1 + k * 512, src + i1 + k * TSV);
+                    cp_async16_tma(base + gd0 + k * 512, src + i0 + k * TSV);
+                    cp_async16_tma(base + gd1 + k * 512, src + i1 + k * TSV);
                     if (GATHER_Y) {
-                        if (!(SKIPM & 0x100)) cp_async16_tma(base + gd2 + k * 512, src + i2 + k * TSV);
-                        if (!(SKIPM & 0x200)) cp_async16_tma(base + gd3 + k * 512, src + i3 + k * TSV);
+                        cp_async16_tma(base + gd2 + k * 512, src + i2 + k * TSV);
+                        cp_async16_tma(base + gd3 + k * 512, src + i3 + k * TSV);
                     }
                 }
                 cp_async_mbar_arrive_noinc(full);
@@ -891,7 +881,6 @@ static dwf_status launch_tma_t(dwf_ctx* c, const TmaArgs& a, const CUtensorMap* 
         DWF_CUDA_CHECK(c, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     TmaState* s = (TmaState*)c->tma;
     int grid = s->num_sms * MINB;
-    if (c->dhop_grid > 0) grid = c->dhop_grid;
     if (grid > c->g.ntiles) grid = c->g.ntiles;
     if (grid_out) *grid_out = grid;
     kern<<<grid, 128 + 128 * TPS, smem, c->stream>>>(a, maps[0], maps[1], maps[2]);
@@ -916,9 +905,6 @@ static dwf_status fill_args(dwf_ctx* c, TmaArgs& a, void* out, const void* in, i
     a.order = s->order;
     a.counters = s->counters;
     a.mode = c->dhop_dynamic;
-#ifdef DWF_PROBE
-    a.skip = c->dhop_skip;
-#endif
     a.dagger = dagger;
     a.epi.mode = EPI_NONE;
     return DWF_OK;

@@ -186,6 +186,7 @@ __global__ void __launch_bounds__(128) op5_kernel(int Ls_rt, int TS, unsigned nv
 // init: p <- r, ap = A p, x untouched.  alpha = sc[slot_c]/sc[slot_d], beta = sc[slot_cn]/sc[slot_c] of the thread's
 // right-hand side (blockIdx.y).  A system whose stopping test fired at an EARLIER iteration (conv[rhs] in [0, iter)) is
 // frozen: the host runs one iteration ahead of the residuals it has read, and other systems of a batch may still iterate.
+// A frozen system keeps x and p; its ap is set to zero (see below) and cg_r_kernel leaves its r alone.
 template <typename R>
 __global__ void __launch_bounds__(128) cg_xp_kernel(int Ls, int TS, unsigned nvec_site, typename V5<R>::V* __restrict__ x,
                                                     typename V5<R>::V* __restrict__ p,
@@ -198,15 +199,21 @@ __global__ void __launch_bounds__(128) cg_xp_kernel(int Ls, int TS, unsigned nve
     const unsigned gid = blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= nvec_site) return;
     const int rhs = blockIdx.y;
-    if (!init) {
-        const int cv = conv[rhs];
-        if (cv >= 0 && cv < iter) return;
-    }
     const unsigned per_tile = (unsigned)K * TS;
     const unsigned tile = gid / per_tile, j = gid - tile * per_tile;
     const int k = j / TS;
     const bool rev = (k >= K / 2);
     const size_t base = ((size_t)tile * gridDim.y + rhs) * Ls * per_tile + j;
+    if (!init) {
+        const int cv = conv[rhs];
+        if (cv >= 0 && cv < iter) {
+            // frozen: x and p stay.  ap is the buffer the Dhop chain works in, so it holds that chain's last output, not
+            // A p: zero it, the chain of this system then carries zeros (and cg_r skips the system) instead of feeding
+            // its own output back into itself iteration after iteration until it overflows.
+            for (int jj = 0; jj < Ls; ++jj) ap[base + (size_t)jj * per_tile] = zerov((V*)nullptr);
+            return;
+        }
+    }
     R alpha = (R)0, beta = (R)0;
     if (!init) {
         const double cc = sc[slot_c * MAXR + rhs];
@@ -361,12 +368,16 @@ __global__ void __launch_bounds__(128) cg_r_kernel(int Ls, int TS, unsigned nvec
                                                    const typename V5<R>::V* __restrict__ q,
                                                    const typename V5<R>::V* __restrict__ d, const double* __restrict__ sc,
                                                    int slot_c, int slot_d, R bee, R mcee, R yb5, R yc5, R mf,
-                                                   double* __restrict__ partials) {
+                                                   double* __restrict__ partials, const int* __restrict__ conv, int iter) {
     using V = typename V5<R>::V;
     constexpr int K = V5<R>::K;
     const unsigned gid = blockIdx.x * blockDim.x + threadIdx.x;
     double nrm = 0.0;
-    if (gid < nvec_site) {
+    // a system whose stopping test fired at an earlier iteration is frozen (cg_xp_kernel): its chain carries zeros, its
+    // scalars are no longer meaningful (d = 0), r stays as it is and the partial written for it is 0
+    const int cv = conv[blockIdx.y];
+    const bool frozen = (cv >= 0 && cv < iter);
+    if (gid < nvec_site && !frozen) {
         const unsigned per_tile = (unsigned)K * TS;
         const unsigned tile = gid / per_tile, j = gid - tile * per_tile;
         const int k = j / TS;
@@ -411,12 +422,12 @@ dwf_status launch_cg_r(dwf_ctx* c, void* r, const void* q, const void* d, double
     if (prec == DWF_F64)
         cg_r_kernel<double><<<grid, block, 0, c->stream>>>(g.Ls, g.TS, nvec_site, (double2*)r, (const double2*)q,
                                                            (const double2*)d, c->scalars, slot_c, slot_d, bee, -cee,
-                                                           yscale * c->b5, yscale * c->c5, c->mf, c->partials);
+                                                           yscale * c->b5, yscale * c->c5, c->mf, c->partials, c->cg_conv, iter);
     else
         cg_r_kernel<float><<<grid, block, 0, c->stream>>>(g.Ls, g.TS, nvec_site, (float4*)r, (const float4*)q,
                                                           (const float4*)d, c->scalars, slot_c, slot_d, (float)bee,
                                                           (float)-cee, (float)(yscale * c->b5), (float)(yscale * c->c5),
-                                                          (float)c->mf, c->partials);
+                                                          (float)c->mf, c->partials, c->cg_conv, iter);
     c->launches++;
     DWF_CUDA_CHECK(c, cudaGetLastError());
     return launch_reduce(c, gridx, norm_slot, iter);

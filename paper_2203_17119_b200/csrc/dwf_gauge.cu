@@ -67,7 +67,7 @@ dwf_status check_su3(dwf_ctx* c, const double* Ucanon) {
     unsigned long long* w = reinterpret_cast<unsigned long long*>(c->scalars + (size_t)SLOT_T1 * MAXR);
     DWF_CUDA_CHECK(c, cudaMemsetAsync(w, 0, sizeof(*w), c->stream));
     const long long nlinks = 2LL * c->g.Vh * 4;
-    su3_defect_kernel<<<148 * 4, 256, 0, c->stream>>>(Ucanon, nlinks, w);
+    su3_defect_kernel<<<c->num_sms * 4, 256, 0, c->stream>>>(Ucanon, nlinks, w);
     c->launches++;
     double d = 0.0;
     DWF_CUDA_CHECK(c, cudaMemcpyAsync(&d, w, sizeof(d), cudaMemcpyDeviceToHost, c->stream));

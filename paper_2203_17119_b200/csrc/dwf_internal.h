@@ -70,16 +70,9 @@ struct dwf_ctx {
     int cut[4];
     int compress12 = 1;
     int tile_opt[4] = {0, 0, 0, 0};
-    int dhop_sc = 0;       // 0 = library default per precision
-    int dhop_loop_s = 0;
     int dhop_kernel = 0;   // 0 = auto (TMA kernel for 4^4 tiles, else cp.async tile kernel, else generic), 1 = generic, 2 = cp.async tile kernel
-    int dhop_nst = 3;      // ring depth of the pipelined fp32 kernel
-    int dhop_grid = 0;     // CTAs of the persistent TMA kernel (0 = SMs x resident CTAs)
     int fuse = 1;          // Mpc / CG through the Dhop kernel's fused 5-D epilogues when the TMA kernel applies (0: separate op5 kernels)
     int dhop_dynamic = 1;  // TMA kernel tile scheduling: 1 global in-order queue (default), 0 static round-robin (same results: every reduction is per tile)
-    int dhop_skip = 0;     // debug only (traffic attribution): halo regions the TMA kernel does not load
-    int dhop_order = 0;    // tile traversal of the TMA kernel: blob extents in tiles as digits (0 = default), dwf_dhop_tma.cu
-    int dhop_order_axes = 0;   // blob path, fastest-first axis digits
     void* tma = nullptr;   // dwf::TmaState (dwf_dhop_tma.cu), built at dwf_set_gauge for 4^4 tiles
     // tables of the pipelined Dhop kernel (dwf_dhop_pipe.cu), built at dwf_set_gauge
     uint16_t* pipe_nbslot[2] = {nullptr, nullptr};      // [precision]: the two precisions differ in lane order
@@ -91,6 +84,7 @@ struct dwf_ctx {
     int max_restarts = 20;
     cudaStream_t stream = nullptr;
     int device = 0;        // CUDA device the context was created on; every ABI call runs with it current (DeviceGuard)
+    int num_sms = 148;     // cudaDevAttrMultiProcessorCount of that device (dwf_create): grid sizes of the streaming kernels
     bool gauge_set = false;
     bool geom_frozen = false;
     // gauge copies [parity]
@@ -106,7 +100,7 @@ struct dwf_ctx {
     size_t bnd_ws_bytes = 0;
     dwf::Table5 tab[dwf::OP5_COUNT];
     dwf::DevTables dtab;
-    // workspace (allocated lazily, sized for half fields)
+    // solver workspace: 10 half fields per precision, allocated at dwf_set_gauge (ws_alloc_all, dwf_api.cu)
     void* ws64[10] = {};
     void* ws32[10] = {};
     dwf::MsState* ms_state = nullptr;   // multishift CG: device-resident scalar recurrences

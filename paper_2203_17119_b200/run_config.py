@@ -57,7 +57,7 @@ def run(cfg, U, b_np, with_sweeps=True, max_iter=50000, extras=False):
                      "resid_true": info["resid_true"], "seconds": info["seconds"], "launches": info["launches"]}
         del x
     if extras and any(cfg.cut) and all(c == 0 or (d // c) % 2 == 0 for d, c in zip(cfg.dims, cfg.cut)):
-        # the boundary operators R^-1 (one uncut solve) and R (two Dirichlet solves), eqs. 13-14
+        # the boundary operators R^-1 (one uncut solve, eqs. 13-14) and R (two Dirichlet solves, eqs. 9-10)
         phi = g.new_native(A.F64, A.FULL).normal_()
         p = g.domain_project(phi, 2)
         rinv, i1, st1 = g.boundary_op(phi, True, cfg.tol, max_iter, A.CG_MIXED)
