@@ -1,5 +1,5 @@
-"""SURVEY 8f NEXT-1 through the C ABI: the domain and boundary projectors and the paper's boundary operators R (eq. 13) and
-R^-1 (eq. 14) against oracle/boundary.py on small lattices, and the identity R R^-1 = P
+"""SURVEY 8f NEXT-1 through the C ABI: the domain and boundary projectors and the paper's boundary operators R (eqs. 9-10) and
+R^-1 (eqs. 13-14) against oracle/boundary.py on small lattices, and the identity R R^-1 = P
 on the GPU alone at BASELINE configs[1] (c2, 16^4 x 16, two 16^3 x 8 domains)."""
 import numpy as np
 import pytest

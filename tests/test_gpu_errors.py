@@ -42,6 +42,11 @@ def test_aliasing_bad_tolerance_and_late_options(ctx):
     info = api.CgInfo()
     st = g.lib.dwf_cg(g._h, g._p(g.new_native()), g._p(a), -1.0, 10, api.CG_F64, 0, ctypes.byref(info))
     assert st == api.EINVAL
+    full = g.new_native(api.F64, api.FULL).normal_()
+    for fn in (lambda: g.lib.dwf_cg(g._h, g._p(g.new_native()), g._p(a), 1e-8, -1, api.CG_F64, 0, ctypes.byref(info)),
+               lambda: g.lib.dwf_solve(g._h, g._p(g.new_native(api.F64, api.FULL)), g._p(full), 1e-8, -1, api.CG_F64,
+                                       ctypes.byref(info))):
+        assert fn() == api.EINVAL                      # a negative iteration budget is a bad argument everywhere
     with pytest.raises(api.DwfError) as e:
         g.set_option("compress12", 0)                  # layout options are frozen once the gauge field is in
     assert e.value.status == api.ESTATE

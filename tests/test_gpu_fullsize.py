@@ -97,6 +97,26 @@ def test_c4_cg_first_iterations_match_oracle(c4):
     assert abs(info["resid_true"] - true_res) <= 1e-9 * true_res
 
 
+@pytest.mark.parametrize("mode", ["f64", "mixed"])
+def test_c4_converged_solution_certified_by_the_oracle(c4, mode):
+    """BASELINE configs[3]: "red-black CG to 1e-8 fp64" (and the fp32-inner variant) on the headline lattice, run to
+    convergence on the GPU; the oracle then recomputes |b - Mpc^dag Mpc x| / |b| of the returned solution with one
+    application of its own operator (SURVEY 8(d) reading (3)): it must meet the tolerance and confirm the residual the
+    library reports about itself."""
+    A, g, orc, odd, cfg = c4["api"], c4["g"], c4["orc"], c4["odd"], c4["cfg"]
+    tol = cfg.tol
+    assert tol == 1e-8
+    x, info, st = g.cg(g.pack(odd, A.F64, A.ODD), tol, 20000, A.CG_MIXED if mode == "mixed" else A.CG_F64)
+    assert st == A.OK and info["resid_true"] <= tol and info["iters_total"] > 100
+    if mode == "mixed":
+        assert info["iters_inner"] == info["iters_total"] and info["restarts"] >= 1
+    xs = g.unpack(x, A.F64, A.ODD)
+    del x
+    true_res = np.sqrt(orc.norm2(odd - orc.mdagm(xs)) / orc.norm2(odd))
+    assert true_res <= tol * (1 + 1e-6), (true_res, info)
+    assert abs(true_res - info["resid_true"]) <= 1e-6 * true_res, (true_res, info)
+
+
 # ---- BASELINE configs[2] = c3: 24^4 x Ls=16 Moebius, eps = 0.5: Dhop in both precisions, mixed-precision CG to 1e-10
 @pytest.fixture(scope="module")
 def c3(oracle_built):

@@ -142,3 +142,34 @@ def test_batched_edge_cases(case):
         g.cg_mrhs(batched, 17, 1e-9, 10)
     with pytest.raises(A.DwfError):
         g.dhop_mrhs(batched, n, A.FULL)
+
+
+@pytest.mark.parametrize("mode", ["f64", "mixed"])
+def test_system_frozen_long_before_the_rest_of_its_batch(case, mode):
+    """A system whose stopping test fires at once (its initial guess is already the solution) stays frozen while the other
+    systems of the batch run their full course.  On the fused path its Dhop chain then carries zeros and cg_r leaves its
+    residual alone (csrc/dwf_fived.cu: cg_xp_kernel / cg_r_kernel); its x must come out finite, untouched by the others'
+    iterations, and equal to what the single-system solve with the same guess returns, bit for bit."""
+    import torch
+    A, g, n = case["api"], case["g"], case["nrhs"]
+    M = A.CG_MIXED if mode == "mixed" else A.CG_F64
+    tol = 1e-10
+    nat = [g.pack(s, A.F64, A.ODD) for s in case["srcs"]]
+    x_done, i_done, st = g.cg(nat[0], 1e-12, 20000, A.CG_F64)
+    assert st == A.OK
+    guesses = [x_done.clone()] + [torch.zeros_like(nat[0]) for _ in range(n - 1)]
+    x, infos, st = g.cg_mrhs(g.mrhs_gather(nat), n, tol, 20000, M, x=g.mrhs_gather(guesses), use_guess=True)
+    assert st == A.OK
+    xs = g.mrhs_scatter(x, n)
+    assert infos[0]["iters_total"] == 0 and torch.equal(xs[0], x_done)             # never moved
+    assert max(i["iters_total"] for i in infos[1:]) >= 20                            # while the others iterated
+    for j in range(n):
+        assert bool(torch.isfinite(xs[j]).all()), j
+        x1, i1, st1 = g.cg(nat[j], tol, 20000, M, x=guesses[j].clone(), use_guess=True)
+        assert st1 == A.OK
+        if mode == "f64":
+            assert i1["iters_total"] == infos[j]["iters_total"], (j, i1, infos[j])
+            assert torch.equal(x1, xs[j]), j
+        else:
+            assert abs(i1["iters_total"] - infos[j]["iters_total"]) <= max(2, infos[j]["iters_total"] // 50), (j, i1, infos[j])
+        assert infos[j]["resid_true"] <= tol

@@ -121,8 +121,8 @@ def test_R_and_Rinv_eqs_13_14(setup):
     DO, DOb, Dd, Ddb = M[np.ix_(om, om)], M[np.ix_(ob, ob)], M[np.ix_(om, ob)], M[np.ix_(ob, om)]
     X = np.zeros_like(M)
     X[np.ix_(om, om)] = np.linalg.solve(DO, Dd @ np.linalg.solve(DOb, Ddb))
-    R = P - P @ X                                                   # eq. 13
-    Rinv = P - P @ np.linalg.solve(M, Dh)                           # eq. 14
+    R = P - P @ X                                                   # eqs. 9-10
+    Rinv = P - P @ np.linalg.solve(M, Dh)                           # eqs. 13-14
     assert rel(R @ Rinv, P) < 1e-11 and rel(Rinv @ R, P) < 1e-11    # "R R^-1 = P"
     rng = np.random.default_rng(5)
     phi = rng.standard_normal(n) + 1j * rng.standard_normal(n)

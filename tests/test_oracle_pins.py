@@ -346,6 +346,73 @@ def test_cg_vs_dense_solve(U, psi, oracle_built):
     assert info2["iters"] == 0 and info2["converged"]
 
 
+def test_norm2_is_the_plain_sum_of_squares(psi, oracle_built):
+    """orc_norm2 pinned directly: every other pin uses it only in ratios, where a wrong normalisation (a half-summed array,
+    |re|^2 only) would cancel.  numpy's vdot on the same values, both precisions (the fp32 oracle accumulates in fp64, C8)."""
+    _, b = split(psi, DIMS)
+    o64, o32 = Oracle(DIMS, LS, **SHAM), Oracle(DIMS, LS, prec="f32", **SHAM)
+    want = float(np.vdot(b, b).real)
+    assert abs(o64.norm2(b) - want) <= 1e-14 * want
+    b32 = b.astype(np.complex64)
+    want32 = float(np.vdot(b32.astype(np.complex128), b32.astype(np.complex128)).real)
+    assert abs(o32.norm2(b32) - want32) <= 1e-14 * want32
+    e = np.zeros_like(b)
+    e.reshape(-1)[-1] = 3 - 4j                                     # the last element counts, re and im both
+    assert o64.norm2(e) == 25.0 and o64.norm2(np.zeros_like(b)) == 0.0
+
+
+def test_cg_restarts_from_the_true_residual(U, psi, oracle_built):
+    """Reading C8's restart rule, entered for real: at tol = 4e-15 the recurrence residual passes the test while the true
+    residual b - A x (~5e-15 here, fp64 rounding of 160 iterations) does not, so the solve must recompute r = b - A x, go
+    on from the current x, keep counting iterations, and stop once the TRUE residual is below tol.  Checked against the
+    same rule written around numpy's dense Mpc (independent construction, tests/dense_ref.py), and against what holds
+    whatever the rule's details: the answer satisfies the dense system to tol, at least one restart happened, and the
+    restarted solve took more iterations than the recurrence alone asks for (restart_on_true=False)."""
+    par = MOEB
+    o = make(par, U)
+    M = dr.dwf_matrix(U, DIMS, LS, par["M5"], par["mf"], par["b5"], par["c5"])
+    ev, od = dr.parity_index(DIMS, LS)
+    Mpc = M[np.ix_(od, od)] - M[np.ix_(od, ev)] @ np.linalg.solve(M[np.ix_(ev, ev)], M[np.ix_(ev, od)])
+    Mh = Mpc.conj().T
+    _, b = split(psi, DIMS)
+    bv = b.reshape(-1)
+    tol, max_iter = 4e-15, 2000
+    n2 = lambda v: float(np.vdot(v, v).real)
+    bn2 = n2(bv)
+    target = tol * tol * bn2
+    x = np.zeros_like(bv)
+    iters = restarts = 0
+    while True:
+        r = bv - Mh @ (Mpc @ x) if restarts else bv.copy()
+        p, c = r.copy(), n2(r)
+        while c > target and iters < max_iter:
+            q = Mpc @ p
+            alpha = c / n2(q)
+            x += alpha * p
+            r -= alpha * (Mh @ q)
+            cn = n2(r)
+            iters += 1
+            if cn <= target:
+                break
+            p = r + (cn / c) * p
+            c = cn
+        true = np.sqrt(n2(bv - Mh @ (Mpc @ x)) / bn2)
+        if true <= tol or iters >= max_iter:
+            break
+        restarts += 1
+    assert true <= tol and restarts >= 1
+    xo, info = cg(o, b, tol, max_iter)
+    assert info["converged"] and info["restarts"] >= 1
+    assert info["restarts"] == restarts and abs(info["iters"] - iters) <= 2, (info, restarts, iters)
+    # independent of the rule's wording: the dense system is solved to tol, and the reported true residual is the real one
+    dense_true = np.sqrt(n2(bv - Mh @ (Mpc @ xo.reshape(-1))) / bn2)
+    # (to the rounding of evaluating b - A x itself, ~1e-15 relative here: two evaluations differ by that much)
+    assert dense_true <= 1.5 * tol and abs(dense_true - info["resid_true"]) <= 0.5 * tol
+    _, plain = cg(o, b, tol, max_iter, restart_on_true=False)
+    assert plain["restarts"] == 0 and not plain["converged"] and plain["resid_true"] > tol
+    assert info["iters"] > plain["iters"]                          # iterations of all passes are counted
+
+
 def test_multishift_cg_vs_dense_solves(U, psi, oracle_built):
     """NEXT-2: every shifted solution against numpy's dense solve of (Mpc^dag Mpc + sigma) x = b, the matrix built
     from dense blocks (independent of the oracle's loops); one shared iteration count; sigma = 0 reproduces plain CG."""
