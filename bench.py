@@ -156,19 +156,23 @@ def oracle_setup(cfg, dims, U=None, b=None):
 def oracle_workload_baseline(cfg, U, b, iters=1):
     """cpu_baseline of the own arm: the oracle, as it stands, on the WORKLOAD ITSELF (same lattice, gauge field and source
     the GPU step ran on): one Dhop (1 warm-up + 3 repetitions), one Mpc^dag Mpc (1 + 2) and one CG segment of `iters`
-    iteration(s) with |b|^2 and the closing true residual (1 repetition, after the warm-ups above)."""
+    iteration(s) with |b|^2 and the closing true residual (1 warm-up + 2 repetitions, each timed: the value is their mean,
+    the two samples are reported beside it)."""
     from oracle.dwf_oracle import cg
     orc, b = oracle_setup(cfg, cfg.dims, U, b)
     n5h = b.shape[0] * cfg.Ls
     t_dhop = _timed(lambda: orc.dhop(b, 0, False), 1, 3)
     t_mdagm = _timed(lambda: orc.mdagm(b), 1, 2)
-    t_seg = _timed(lambda: cg(orc, b, 1e-300, iters), 0, 1)
+    cg(orc, b, 1e-300, iters)
+    segs = [_timed(lambda: cg(orc, b, 1e-300, iters), 0, 1) for _ in range(2)]
+    t_seg = sum(segs) / len(segs)
     return {"value": segment_flops(n5h, iters) / t_seg / 1e9, "unit": UNIT, "kind": "oracle", "s_per_step": t_seg,
+            "s_per_step_samples": segs,
             "dhop_s": t_dhop, "dhop_gflops": FLOP_DHOP * n5h / t_dhop / 1e9,
             "mdagm_s": t_mdagm, "mdagm_gflops": 2 * FLOP_MPC * n5h / t_mdagm / 1e9,
             "sample": f"the workload itself ({'x'.join(map(str, cfg.dims))} x Ls={cfg.Ls}, the GPU step's gauge field and source): "
-                      f"half-volume Dhop 1+3 repetitions, Mpc^dag Mpc 1+2, one CG segment of {iters} iteration(s) + |b|^2 + closing "
-                      f"true residual (the GPU step runs 10 iterations per segment); oracle built -O3 -march=native -fno-fast-math"}
+                      f"half-volume Dhop 1+3 repetitions, Mpc^dag Mpc 1+2, CG segment of {iters} iteration(s) + |b|^2 + closing "
+                      f"true residual 1+2 (the GPU step runs 10 iterations per segment); oracle built -O3 -march=native -fno-fast-math"}
 
 
 def run_reference(args, cfg):
@@ -216,6 +220,55 @@ def workload_name(cfg):
 
 
 # ------------------------------------------------------------------------------------------------ own arm
+HBM_NOMINAL_GBS = 8000.0          # B200 data sheet (SURVEY 8d asks for the fraction against both HBM figures)
+# Arithmetic instructions of the plain Dhop kernel per 5-D site, from the SASS histogram profiles/r02_sass_hist.md:
+# fp64 2 lanes x 432 DFMA/DADD/DMUL per site-slice, fp32 870 FFMA/FADD/FMUL per site-slice; 1320 flop per site.
+ALU_INST_PER_SITE = {"f64": 864.0, "f32": 870.0}
+ALU_LANES_PER_SM = {"f64": 64, "f32": 128}         # FP64 / FP32 FMA lanes per SM per clock on sm_100
+LIMITER_NOTE = ("sm_latency: the launch time follows the SM clock (ncu at 1.80 GHz against the power-capped clock of the step, "
+                "DESIGN.md 5.1); neither HBM (frac) nor the arithmetic pipe (alu.frac_issue) is saturated")
+
+
+def alu_block(sites, launch_ms, sm_mhz, prec, g):
+    """The ALU side of the roofline ('HBM first, with the plain FP32/FP64 ALUs a close second') at the SM clock
+    sampled during the timed region: frac_issue = arithmetic instructions issued per second / (SMs x lanes x clock),
+    frac_flops = useful flop/s / (SMs x lanes x 2 x clock)."""
+    if not sm_mhz or launch_ms <= 0:
+        return None
+    import torch
+    sms = torch.cuda.get_device_properties(g.device).multi_processor_count
+    lanes = ALU_LANES_PER_SM[prec]
+    t = launch_ms * 1e-3
+    inst_peak = sms * lanes * sm_mhz * 1e6
+    return {"sm_count": sms, "lanes_per_sm": lanes, "inst_per_site": ALU_INST_PER_SITE[prec],
+            "peak_gflops_at_clock": 2 * inst_peak / 1e9, "frac_issue": ALU_INST_PER_SITE[prec] * sites / t / inst_peak,
+            "frac_flops": FLOP_DHOP * sites / t / (2 * inst_peak)}
+
+
+def ev_median(torch, fn, warm=10, min_reps=100, min_s=1.0, max_reps=2000):
+    """SURVEY 8d 'GPU timing': >= 10 warm-ups, then one CUDA-event pair per repetition until >= 100 repetitions or >= 1 s of
+    kernel time; returns (median ms, first-repetition ms after the warm-ups, repetitions)."""
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    times, total = [], 0.0
+    while len(times) < max_reps and (len(times) < min_reps and total < min_s * 1e3):
+        batch = []
+        for _ in range(10):
+            s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            s.record()
+            fn()
+            e.record()
+            batch.append((s, e))
+        torch.cuda.synchronize()
+        for s, e in batch:
+            t = s.elapsed_time(e)
+            times.append(t)
+            total += t
+    st = sorted(times)
+    return st[len(st) // 2], times[0], len(times)
+
+
 def ev_time(torch, fn, reps):
     s, e = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
@@ -293,13 +346,18 @@ def run_dwf(args, cfg):
     dhop_avg_ms = dhop_ms / max(dhop_n, 1)
     dhop_bytes = dhop_bytes_total / max(dhop_n, 1)
     achieved = dhop_bytes / (dhop_avg_ms * 1e-3) / 1e9
-    traffic64, traffic_src = static_traffic("dhop_f64")
+    traffic64, traffic_src, stale64 = static_traffic("dhop_f64")
+    sm_mhz = (clocks or {}).get("sm_mhz") or None
+    sites = n5h                                            # 5-D sites one half-volume launch writes
     roofline = {"bound": "hbm", "dtype": "f64",
                 "kernel": "dhop_tma_kernel<double> (half-volume, 12-real links; per CG iteration 3 plain launches + 1 with the fused Mee epilogue)",
                 "achieved": achieved, "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s", "frac": achieved / hbm_peak,
                 "traffic": traffic64, "traffic_source": traffic_src, "algorithmic_bytes_per_launch": dhop_bytes,
                 "avg_launch_ms": dhop_avg_ms, "launches_timed": int(dhop_n), "share_of_step": dhop_ms / ms if ms > 0 else None,
-                "gflops": FLOP_DHOP * n5h / (dhop_avg_ms * 1e-3) / 1e9}
+                "gflops": FLOP_DHOP * n5h / (dhop_avg_ms * 1e-3) / 1e9,
+                "traffic_stale": stale64, "frac_nominal": achieved / HBM_NOMINAL_GBS, "peak_nominal": HBM_NOMINAL_GBS,
+                "sm_mhz": sm_mhz, "alu": alu_block(sites, dhop_avg_ms, sm_mhz, "f64", g),
+                "limiter": LIMITER_NOTE}
 
     # ---- the same per-launch event timing for the fp32 kernel, inside a long fp32 step with the CG's launch mix (3 plain
     # + 1 fused Dhop per Mpc^dag Mpc): Chebyshev recurrences of Mpc^dag Mpc in fp32 (dwf_chebyshev, order = 2 x cg-iters)
@@ -315,12 +373,15 @@ def run_dwf(args, cfg):
     g.set_option("time_dhop", 0)
     del src32, out32
     avg32, b32 = ms32 / max(n32, 1), by32 / max(n32, 1)
-    traffic32, traffic32_src = static_traffic("dhop_f32")
+    traffic32, traffic32_src, stale32 = static_traffic("dhop_f32")
     roofline_f32 = {"bound": "hbm", "dtype": "f32", "kernel": "dhop_tma_kernel<float> (same launch mix, inside fp32 Chebyshev steps of Mpc^dag Mpc)",
                     "achieved": b32 / (avg32 * 1e-3) / 1e9, "peak": hbm_peak, "peak_source": peak_src, "unit": "GB/s",
                     "frac": b32 / (avg32 * 1e-3) / 1e9 / hbm_peak, "traffic": traffic32, "traffic_source": traffic32_src,
                     "algorithmic_bytes_per_launch": b32, "avg_launch_ms": avg32, "launches_timed": int(n32),
-                    "gflops": FLOP_DHOP * n5h / (avg32 * 1e-3) / 1e9}
+                    "gflops": FLOP_DHOP * n5h / (avg32 * 1e-3) / 1e9,
+                    "traffic_stale": stale32, "frac_nominal": b32 / (avg32 * 1e-3) / 1e9 / HBM_NOMINAL_GBS,
+                    "peak_nominal": HBM_NOMINAL_GBS, "sm_mhz": sm_mhz, "alu": alu_block(sites, avg32, sm_mhz, "f32", g),
+                    "limiter": LIMITER_NOTE}
 
     # ---- e2e: the same step through the C ABI with pinned HOST buffers
     b_host = torch.from_numpy(np.ascontiguousarray(b_np).view(np.float64).reshape(-1)).pin_memory()
@@ -348,12 +409,17 @@ def run_dwf(args, cfg):
                        "l2": "inputs_larger_than_L2 (each half field 1.2 GB, gauge 0.4 GB per parity)", "parallelism": f"replicas x{world}: one seeded {cfg.name} subdomain per GPU, no data-path collective"},
             "clocks": clocks, "gpu_launches": int(launches), "roofline": roofline, "roofline_f32": roofline_f32, "e2e": e2e}
 
+    cpu_leg = rank == 0 and world == 1 and not args.no_cpu
+    xs = {} if cpu_leg else None
     if rank == 0 and not args.no_extras:
         line["sweeps"] = sweeps(torch, g, A, cfg, hbm_peak)
-        line["cg"] = cg_solutions(g, A, b, cfg, args)
-    if rank == 0 and world == 1 and not args.no_cpu:
+        line["cg"] = cg_solutions(g, A, b, cfg, args, keep=xs)
+    if cpu_leg:
         cpu = host_cpu()
         line["cpu_baseline"] = {**oracle_workload_baseline(cfg, U, b_np, args.ref_iters), "cores": cpu["threads"], **cpu}
+        if xs:                                                              # the converged solves, certified by the oracle
+            for name, res in oracle_residuals(cfg, U, b_np, xs).items():
+                line["cg"][name]["resid_true_oracle"] = res
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -361,51 +427,74 @@ def run_dwf(args, cfg):
         print(json.dumps(line), flush=True)
 
 
+def kernel_source_sha():
+    """sha256 (first 16 hex digits) of csrc/dwf_dhop_tma.cu with // comments and blank lines removed: the fingerprint
+    profiles/dhop_traffic.csv stores for the kernel source its ncu capture was taken from (there is no .git on the GPU box)."""
+    import hashlib
+    import re
+    txt = open(os.path.join(ROOT, "paper_2203_17119_b200", "csrc", "dwf_dhop_tma.cu")).read()
+    lines = [re.sub(r"//.*$", "", ln).rstrip() for ln in txt.splitlines()]
+    return hashlib.sha256("\n".join(ln for ln in lines if ln.strip()).encode()).hexdigest()[:16]
+
+
 def static_traffic(kernel):
     """ncu DRAM bytes per launch of the Dhop kernels: NOT measured in this run -- read from the committed ncu summary
-    (profiles/dhop_traffic.csv names the capture and the commit it was taken at); null when the file has no row."""
+    (profiles/dhop_traffic.csv names the capture and the fingerprint of the kernel source it was taken from); null when the
+    file has no row.  Returns (bytes, source description, stale): stale = the kernel source has changed since the capture."""
     tp = os.path.join(ROOT, "profiles", "dhop_traffic.csv")
     if os.path.exists(tp):
         import csv
         for row in csv.DictReader(open(tp)):
             if row["kernel"] == kernel:
-                return float(row["dram_bytes_per_launch"]), f"static: profiles/dhop_traffic.csv ({row.get('capture', 'ncu --set full')})"
-    return None, "none"
+                stale = row.get("source_sha", "") != kernel_source_sha()
+                return (float(row["dram_bytes_per_launch"]),
+                        f"static: profiles/dhop_traffic.csv ({row.get('capture', 'ncu --set full')}; kernel source {row.get('source_sha', '?')})", stale)
+    return None, "none", None
 
 
 def sweeps(torch, g, A, cfg, hbm_peak):
-    """Kernel-alone sweeps (CUDA events, 3 warm-ups): full-volume Dhop and Mpc^dag Mpc in fp32 and fp64."""
+    """Kernel-alone sweeps (CUDA events, >= 10 warm-ups, >= 100 repetitions or >= 1 s, median): full-volume Dhop
+    and Mpc^dag Mpc in fp32 and fp64."""
     out = {}
     n5h = (cfg.V4 // 2) * cfg.Ls
     for prec, name, B in ((A.F32, "f32", 4), (A.F64, "f64", 8)):
         src = g.new_native(prec, A.FULL).normal_()
         dst = g.new_native(prec, A.FULL)
-        for _ in range(3):
-            g.dhop(src, A.FULL, False, prec, out=dst)
-        ms = ev_time(torch, lambda: g.dhop(src, A.FULL, False, prec, out=dst), 20)
+        ms, first, reps = ev_median(torch, lambda: g.dhop(src, A.FULL, False, prec, out=dst))
         by = 2 * (n5h * 48 * B + (cfg.V4 // 2) * 8 * 12 * B)
         out[f"dhop_{name}"] = {"ms_full_volume": ms, "gflops": FLOP_DHOP * 2 * n5h / ms / 1e6, "gbs": by / ms / 1e6,
-                               "frac_hbm": by / ms / 1e6 / hbm_peak}
+                               "frac_hbm": by / ms / 1e6 / hbm_peak, "frac_hbm_nominal": by / ms / 1e6 / HBM_NOMINAL_GBS,
+                               "timing": f"median of {reps} repetitions after 10 warm-ups", "ms_first_repetition": first}
         so, do = src[: src.numel() // 2], dst[: dst.numel() // 2]
-        for _ in range(3):
-            g.mdagm(so, prec, out=do)
-        ms = ev_time(torch, lambda: g.mdagm(so, prec, out=do), 10)
+        ms, first, reps = ev_median(torch, lambda: g.mdagm(so, prec, out=do))
         by = 2 * (5 * n5h * 24 * B + 2 * (cfg.V4 // 2) * 8 * 12 * B)      # fused minimum 5 S_h + 2 G_h per Mpc
         out[f"mdagm_{name}"] = {"ms": ms, "gflops": 2 * FLOP_MPC * n5h / ms / 1e6, "gbs_fused_minimum": by / ms / 1e6,
-                                "frac_hbm_fused_minimum": by / ms / 1e6 / hbm_peak}
+                                "frac_hbm_fused_minimum": by / ms / 1e6 / hbm_peak,
+                                "timing": f"median of {reps} repetitions after 10 warm-ups", "ms_first_repetition": first}
         del src, dst
     return out
 
 
-def cg_solutions(g, A, b, cfg, args):
-    """red-black CG time-to-solution on the workload (fp64 and fp32-inner/fp64-outer), once each."""
+def cg_solutions(g, A, b, cfg, args, keep=None):
+    """red-black CG time-to-solution on the workload (fp64 and fp32-inner/fp64-outer), once each.  keep: dict that receives
+    the canonical host copy of each solution (for the CPU leg's residual recompute)."""
     out = {}
     for mode, name in ((A.CG_F64, "f64"), (A.CG_MIXED, "mixed")):
         x, info, st = g.cg(b, cfg.tol, args.max_iter, mode)
         out[name] = {"tol": cfg.tol, "status": int(st), "iters": info["iters_total"], "restarts": info["restarts"],
                      "resid_true": info["resid_true"], "time_to_solution_s": info["seconds"], "launches": info["launches"]}
+        if keep is not None:
+            keep[name] = g.unpack(x, A.F64, A.ODD)
         del x
     return out
+
+
+def oracle_residuals(cfg, U, b, xs):
+    """CPU leg (SURVEY 8d reading (3)): the oracle recomputes |b - Mpc^dag Mpc x| / |b| of the GPU's converged solutions with
+    one application of its own operator each."""
+    orc, b = oracle_setup(cfg, cfg.dims, U, b)
+    bn2 = orc.norm2(b)
+    return {name: float(np.sqrt(orc.norm2(b - orc.mdagm(x)) / bn2)) for name, x in xs.items()}
 
 
 def main():
